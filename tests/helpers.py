@@ -1,0 +1,136 @@
+"""Test-side helpers written independently of oracle/ and of the CUDA path.
+
+Everything here is a restatement, in numpy / exact rational arithmetic, of a
+definition in PAPER.md or of a reading in DESIGN.md; it is what the oracle is
+pinned against.
+"""
+from __future__ import annotations
+
+from fractions import Fraction
+
+import numpy as np
+
+
+# ---- exact fp32 helpers ----------------------------------------------------
+def round_f32(x: Fraction) -> np.float32:
+    """Round an exact rational to the nearest fp32 (ties to even), no double rounding."""
+    if x == 0:
+        return np.float32(0.0)
+    c = np.float32(float(x))
+    cands = {c, np.nextafter(c, np.float32(np.inf)), np.nextafter(c, np.float32(-np.inf))}
+    best = None
+    for v in cands:
+        if not np.isfinite(v):
+            continue
+        err = abs(Fraction(float(v)) - x)
+        even = (int(np.float32(v).view(np.uint32)) & 1) == 0
+        key = (err, 0 if even else 1)
+        if best is None or key < best[0]:
+            best = (key, v)
+    return np.float32(best[1])
+
+
+def fmaf_exact(a, b, c) -> np.float32:
+    return round_f32(Fraction(float(a)) * Fraction(float(b)) + Fraction(float(c)))
+
+
+def member_accepts(p, c, s2, th2) -> bool:
+    """fp32 opening test in the exact operation order of DESIGN.md (reading O5)."""
+    f = np.float32
+    dx, dy, dz = f(p[0]) - f(c[0]), f(p[1]) - f(c[1]), f(p[2]) - f(c[2])
+    d2 = fmaf_exact(dz, dz, fmaf_exact(dy, dy, f(dx * dx)))
+    return bool(f(s2) < f(f(th2) * d2))
+
+
+# ---- pair terms, vectorised, written from Eq. 11 / Eq. 12 -------------------
+def pair_terms(rk, uk, rj, uj):
+    """h_kj (Eq. 11) and f_kj (Eq. 12); broadcasting numpy fp64."""
+    rho = np.asarray(rk, float) - np.asarray(rj, float)
+    uk = np.asarray(uk, float)
+    uj = np.asarray(uj, float)
+    r = np.sqrt((rho * rho).sum(-1, keepdims=True))
+    a = (uj * rho).sum(-1, keepdims=True)
+    b = (uk * rho).sum(-1, keepdims=True)
+    c = (uj * uk).sum(-1, keepdims=True)
+    h = (3 * rho * a - uj * r**2) / r**5
+    f = 3 * (rho * c + uk * a + uj * b) / r**5 - 15 * rho * a * b / r**7
+    return h, f
+
+
+def allpairs_numpy(pos, mom):
+    pos = np.asarray(pos, np.float64)
+    mom = np.asarray(mom, np.float64)
+    N = len(pos)
+    H = np.zeros((N, 3))
+    F = np.zeros((N, 3))
+    for k in range(N):
+        m = np.arange(N) != k
+        h, f = pair_terms(pos[k], mom[k], pos[m], mom[m])
+        H[k] = h.sum(0)
+        F[k] = f.sum(0)
+    return H, F
+
+
+# ---- tree by brute-force prefix grouping (reading O3) -----------------------
+def morton_keys_numpy(pos):
+    """30-bit keys, fp32 arithmetic in the order inv=fl(1024/S); q=floor(fl(fl(p-lo)*inv))."""
+    pos = np.asarray(pos, np.float32)
+    lo = pos.min(0)
+    hi = pos.max(0)
+    S = np.float32((hi - lo).astype(np.float32).max())
+    if not S > 0:
+        S = np.float32(1.0)
+    inv = np.float32(np.float32(1024.0) / S)
+    d = (pos - lo).astype(np.float32)
+    g = (d * inv).astype(np.float32)
+    q = np.minimum(np.floor(g).astype(np.int64), 1023)
+    key = np.zeros(len(pos), np.int64)
+    for b in range(10):
+        key |= ((q[:, 0] >> b) & 1) << (3 * b + 2)
+        key |= ((q[:, 1] >> b) & 1) << (3 * b + 1)
+        key |= ((q[:, 2] >> b) & 1) << (3 * b)
+    return key.astype(np.uint32), lo, S
+
+
+def brute_tree(pos, nleaf=1):
+    """Canonical node list [(first, level, prefix, count, is_leaf)] by grouping sorted keys by prefix."""
+    key, lo, S = morton_keys_numpy(pos)
+    perm = np.argsort(key, kind="stable")
+    sk = key[perm].astype(np.int64)
+    N = len(sk)
+    nodes = []
+    internal = {(0, 0)} if N > nleaf else set()
+    nodes.append((0, 0, 0, N, 0 if N > nleaf else 1))
+    for level in range(1, 11):
+        shift = 3 * (10 - level)
+        pref = sk >> shift
+        vals, first, count = np.unique(pref, return_index=True, return_counts=True)
+        new_internal = set()
+        for v, f0, c in zip(vals, first, count):
+            if (level - 1, int(v) >> 3) not in internal:
+                continue
+            leaf = not (c > nleaf and level < 10)
+            nodes.append((int(f0), level, int(v), int(c), 1 if leaf else 0))
+            if not leaf:
+                new_internal.add((level, int(v)))
+        internal |= new_internal
+    nodes.sort(key=lambda t: (t[0], t[1]))
+    return nodes, sk.astype(np.uint32), perm, lo, S
+
+
+def canonical_from_oracle(tree):
+    nd = tree.nodes()
+    return [(int(a), int(b), int(c), int(d), int(e)) for a, b, c, d, e in
+            zip(nd["first"], nd["level"], nd["prefix"], nd["count"], nd["is_leaf"])]
+
+
+# ---- error metric of DESIGN.md ---------------------------------
+def rel_err(x, ref):
+    """Per-particle relative L2 error with the 1e-3*rms floor; returns (max, median, p99, global)."""
+    x = np.asarray(x, np.float64)
+    ref = np.asarray(ref, np.float64)
+    nr = np.linalg.norm(ref, axis=1)
+    rms = np.sqrt((nr**2).mean())
+    e = np.linalg.norm(x - ref, axis=1) / np.maximum(nr, 1e-3 * rms)
+    glob = np.linalg.norm(x - ref) / np.linalg.norm(ref)
+    return float(e.max()), float(np.median(e)), float(np.percentile(e, 99)), float(glob)
