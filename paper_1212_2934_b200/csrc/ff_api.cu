@@ -1,0 +1,278 @@
+// ff_api.cu -- the C ABI of include/ff.h: context, workspace carve-up, phase orchestration.
+#include <math.h>
+#include <new>
+
+#include "ff_internal.cuh"
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// One pass over the workspace layout; with base == nullptr it only measures.
+static size_t carve(ff_ctx* c, char* base, int64_t N)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> char* {
+        char* p = base ? base + off : nullptr;
+        off += align_up(bytes);
+        return p;
+    };
+    size_t n = (size_t)N;
+    size_t cap = 5 * n + 8;                                  // <= N/2 internal cells on each of 10 levels
+    size_t sort_tiles = (n + FF_SORT_TILE - 1) / FF_SORT_TILE;
+    size_t scan_tiles = (n + FF_SCAN_TILE - 1) / FF_SCAN_TILE;
+    char* p;
+    p = take(sizeof(ff_globals));                 if (c) c->g = (ff_globals*)p;
+    for (int b = 0; b < 2; ++b) {
+        p = take(n * 4);                          if (c) c->key[b] = (uint32_t*)p;
+        p = take(n * 4);                          if (c) c->idx[b] = (uint32_t*)p;
+    }
+    p = take(n * 16);                             if (c) c->pos_s = (float4*)p;
+    p = take(n * 16);                             if (c) c->mom_s = (float4*)p;
+    p = take(n * 4);                              if (c) c->leaf_count = (int32_t*)p;
+    p = take(n * 4);                              if (c) c->cell_base = (int32_t*)p;
+    p = take((scan_tiles + 1) * 4);               if (c) c->scan_blk = (uint32_t*)p;
+    p = take(sort_tiles * FF_RADIX * 4);          if (c) c->sort_hist = (uint32_t*)p;
+    p = take(cap * 4);                            if (c) c->cell_first = (int32_t*)p;
+    p = take(cap * 4);                            if (c) c->cell_end = (int32_t*)p;
+    p = take(cap * 4);                            if (c) c->cell_level = (int32_t*)p;
+    p = take(cap * 32);                           if (c) c->cell_child = (int32_t*)p;
+    p = take(cap * 16);                           if (c) c->cell_centre = (float4*)p;
+    p = take(cap * 16);                           if (c) c->cell_moment = (float4*)p;
+    p = take(cap * 24);                           if (c) c->cell_sum_u = (double*)p;
+    p = take(cap * 24);                           if (c) c->cell_sum_p = (double*)p;
+    p = take((size_t)FF_DIRECT_SPLIT_ELEMS * 48); if (c) c->direct_part = (double*)p;
+    p = take(n * 12);                             if (c) c->stage_pos = (float*)p;
+    p = take(n * 12);                             if (c) c->stage_mom = (float*)p;
+    p = take(n * 12);                             if (c) c->stage_H = (float*)p;
+    p = take(n * 12);                             if (c) c->stage_F = (float*)p;
+    p = take(n * 12);                             if (c) c->step_fsr = (float*)p;
+    if (c) c->cell_cap = (int64_t)cap;
+    return off;
+}
+
+extern "C" size_t ff_workspace_bytes(int64_t N)
+{
+    if (N <= 0 || N > FF_MAX_N) return 0;
+    return carve(nullptr, nullptr, N);
+}
+
+extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, size_t workspace_bytes)
+{
+    if (!out) return FF_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (N <= 0 || N > FF_MAX_N || !(theta >= 0.0f) || isinf(theta)) return FF_ERR_INVALID_ARG;
+    size_t need = ff_workspace_bytes(N);
+    if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 255)) return FF_ERR_WORKSPACE;
+    ff_ctx* c = new (std::nothrow) ff_ctx;
+    if (!c) return FF_ERR_INVALID_ARG;
+    memset(c, 0, sizeof(*c));
+    c->N = N; c->theta = theta; c->nleaf = 1;
+    c->ws = (char*)workspace; c->ws_bytes = workspace_bytes;
+    carve(c, c->ws, N);
+    cudaError_t e = cudaGetDevice(&c->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
+    for (int ph = 0; e == cudaSuccess && ph < FF_N_PHASES; ++ph)
+        for (int k = 0; e == cudaSuccess && k < 2; ++k) e = cudaEventCreate(&c->ev[ph][k]);
+    if (e == cudaSuccess) e = cudaMemset(c->g, 0, sizeof(ff_globals));
+    if (e != cudaSuccess) { delete c; return FF_ERR_CUDA; }
+    *out = c;
+    return FF_OK;
+}
+
+extern "C" int ff_destroy(ff_ctx* c)
+{
+    if (!c) return FF_ERR_INVALID_ARG;
+    cudaStreamSynchronize(c->stream);
+    for (int ph = 0; ph < FF_N_PHASES; ++ph)
+        for (int k = 0; k < 2; ++k) if (c->ev[ph][k]) cudaEventDestroy(c->ev[ph][k]);
+    delete c;
+    return FF_OK;
+}
+
+extern "C" int ff_set_stream(ff_ctx* c, void* cuda_stream)
+{
+    if (!c) return FF_ERR_INVALID_ARG;
+    c->stream = (cudaStream_t)cuda_stream;
+    return FF_OK;
+}
+
+extern "C" int ff_set_option(ff_ctx* c, int key, double value)
+{
+    if (!c) return FF_ERR_INVALID_ARG;
+    switch (key) {
+    case FF_OPT_THETA:
+        if (!(value >= 0.0) || isinf(value)) return FF_ERR_INVALID_ARG;
+        c->theta = (float)value;
+        return FF_OK;
+    case FF_OPT_NLEAF:
+        if (!(value >= 1.0) || value > 1e9) return FF_ERR_INVALID_ARG;
+        c->nleaf = (int)value;
+        c->tree_built = 0;
+        return FF_OK;
+    case FF_OPT_COUNTERS: c->count_enabled = value != 0.0; return FF_OK;
+    case FF_OPT_TIMING: c->timing_enabled = value != 0.0; return FF_OK;
+    default: return FF_ERR_INVALID_ARG;
+    }
+}
+
+extern "C" int ff_build_tree(ff_ctx* c, const float* pos, int64_t n)
+{
+    if (!c || !pos || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
+    c->n = n;
+    c->tree_built = 0;
+    c->moments_valid = 0;
+    int rc;
+    ff_phase_begin(c, FF_PH_BBOX_KEYS);
+    if ((rc = ff_launch_bbox_keys(c, pos)) != FF_OK) return rc;
+    ff_phase_end(c, FF_PH_BBOX_KEYS);
+    ff_phase_begin(c, FF_PH_SORT);
+    if ((rc = ff_launch_sort(c, pos)) != FF_OK) return rc;
+    ff_phase_end(c, FF_PH_SORT);
+    ff_phase_begin(c, FF_PH_BUILD);
+    if ((rc = ff_launch_build(c)) != FF_OK) return rc;
+    ff_phase_end(c, FF_PH_BUILD);
+    c->tree_built = 1;
+    return FF_OK;
+}
+
+extern "C" int ff_eval_bh(ff_ctx* c, const float* pos, const float* mom, float* H_out, float* F_out)
+{
+    if (!c || !pos || !mom) return FF_ERR_INVALID_ARG;
+    if (!c->tree_built) return FF_ERR_NO_TREE;
+    int rc;
+    ff_phase_begin(c, FF_PH_MOMENTS);
+    if ((rc = ff_launch_gather_mom(c, mom)) != FF_OK) return rc;
+    if ((rc = ff_launch_moments(c)) != FF_OK) return rc;
+    ff_phase_end(c, FF_PH_MOMENTS);
+    c->moments_valid = 1;
+    ff_phase_begin(c, FF_PH_WALK);
+    if ((rc = ff_launch_walk(c, H_out, F_out)) != FF_OK) return rc;
+    ff_phase_end(c, FF_PH_WALK);
+    return FF_OK;
+}
+
+extern "C" int ff_eval_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n, float* H_out, float* F_out)
+{
+    if (!c || !pos || !mom || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
+    ff_phase_begin(c, FF_PH_DIRECT);
+    int rc = ff_launch_direct(c, pos, mom, n, H_out, F_out);
+    if (rc != FF_OK) return rc;
+    ff_phase_end(c, FF_PH_DIRECT);
+    return FF_OK;
+}
+
+static int host_roundtrip(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h, bool bh)
+{
+    if (!c || !pos_h || !mom_h || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
+    size_t bytes = (size_t)n * 12;
+    FF_CUDA(c, cudaMemcpyAsync(c->stage_pos, pos_h, bytes, cudaMemcpyHostToDevice, c->stream));
+    FF_CUDA(c, cudaMemcpyAsync(c->stage_mom, mom_h, bytes, cudaMemcpyHostToDevice, c->stream));
+    int rc;
+    if (bh) {
+        if ((rc = ff_build_tree(c, c->stage_pos, n)) != FF_OK) return rc;
+        if ((rc = ff_eval_bh(c, c->stage_pos, c->stage_mom, H_h ? c->stage_H : nullptr, F_h ? c->stage_F : nullptr)) != FF_OK) return rc;
+    } else {
+        if ((rc = ff_eval_direct(c, c->stage_pos, c->stage_mom, n, H_h ? c->stage_H : nullptr, F_h ? c->stage_F : nullptr)) != FF_OK) return rc;
+    }
+    if (H_h) FF_CUDA(c, cudaMemcpyAsync(H_h, c->stage_H, bytes, cudaMemcpyDeviceToHost, c->stream));
+    if (F_h) FF_CUDA(c, cudaMemcpyAsync(F_h, c->stage_F, bytes, cudaMemcpyDeviceToHost, c->stream));
+    FF_CUDA(c, cudaStreamSynchronize(c->stream));
+    return FF_OK;
+}
+
+extern "C" int ff_eval_bh_host(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h)
+{
+    return host_roundtrip(c, pos_h, mom_h, n, H_h, F_h, true);
+}
+
+extern "C" int ff_eval_direct_host(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h)
+{
+    return host_roundtrip(c, pos_h, mom_h, n, H_h, F_h, false);
+}
+
+extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n,
+                       const ff_step_params* p, uint64_t step_index)
+{
+    if (!c || !pos || !vel || !mom || !angvel || !p || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
+    if (!(p->dtau > 0.0f)) return FF_ERR_INVALID_ARG;
+    int rc;
+    if ((rc = ff_build_tree(c, pos, n)) != FF_OK) return rc;
+    if ((rc = ff_eval_bh(c, pos, mom, c->stage_H, c->stage_F)) != FF_OK) return rc;
+    ff_phase_begin(c, FF_PH_STEP);
+    if ((rc = ff_launch_step(c, pos, vel, mom, angvel, n, p, step_index)) != FF_OK) return rc;
+    ff_phase_end(c, FF_PH_STEP);
+    c->tree_built = 0;                // positions moved: the tree no longer matches
+    return FF_OK;
+}
+
+extern "C" int ff_get_tree(ff_ctx* c, ff_tree_view* out)
+{
+    if (!c || !out) return FF_ERR_INVALID_ARG;
+    if (!c->tree_built) return FF_ERR_NO_TREE;
+    FF_CUDA(c, cudaStreamSynchronize(c->stream));
+    ff_globals g;
+    FF_CUDA(c, cudaMemcpy(&g, c->g, sizeof(g), cudaMemcpyDeviceToHost));
+    if (g.error) return g.error;
+    memset(out, 0, sizeof(*out));
+    out->n = c->n; out->n_cells = g.n_cells; out->nleaf = c->nleaf;
+    out->lo[0] = g.lo[0]; out->lo[1] = g.lo[1]; out->lo[2] = g.lo[2]; out->S = g.S;
+    out->key = c->key[0]; out->perm = c->idx[0];
+    out->pos_sorted = (const float*)c->pos_s; out->mom_sorted = (const float*)c->mom_s;
+    out->cell_first = c->cell_first; out->cell_end = c->cell_end; out->cell_level = c->cell_level;
+    out->child = c->cell_child; out->leaf_count = c->leaf_count;
+    out->cell_centre = (const float*)c->cell_centre; out->cell_moment = (const float*)c->cell_moment;
+    return FF_OK;
+}
+
+extern "C" int ff_get_timings(ff_ctx* c, float ms[FF_N_PHASES])
+{
+    if (!c || !ms) return FF_ERR_INVALID_ARG;
+    FF_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int ph = 0; ph < FF_N_PHASES; ++ph) {
+        ms[ph] = 0.0f;
+        if (c->ev_valid[ph]) {
+            FF_CUDA(c, cudaEventElapsedTime(&ms[ph], c->ev[ph][0], c->ev[ph][1]));
+            c->ev_valid[ph] = 0;
+        }
+    }
+    return FF_OK;
+}
+
+extern "C" int ff_get_counters(ff_ctx* c, uint64_t* n_cell, uint64_t* n_particle, uint64_t* n_mac_tests)
+{
+    if (!c) return FF_ERR_INVALID_ARG;
+    FF_CUDA(c, cudaStreamSynchronize(c->stream));
+    unsigned long long v[3];
+    FF_CUDA(c, cudaMemcpy(v, c->g->counters, sizeof(v), cudaMemcpyDeviceToHost));
+    if (n_cell) *n_cell = v[0];
+    if (n_particle) *n_particle = v[1];
+    if (n_mac_tests) *n_mac_tests = v[2];
+    return FF_OK;
+}
+
+extern "C" int ff_get_launch_count(ff_ctx* c, uint64_t* launches)
+{
+    if (!c || !launches) return FF_ERR_INVALID_ARG;
+    *launches = c->launches;
+    return FF_OK;
+}
+
+extern "C" int ff_measure_fp32_peak(ff_ctx* c, int iters, double* tflops)
+{
+    if (!c || !tflops) return FF_ERR_INVALID_ARG;
+    return ff_launch_fp32_peak(c, iters, tflops);
+}
+
+extern "C" const char* ff_error_string(int code)
+{
+    switch (code) {
+    case FF_OK: return "ok";
+    case FF_ERR_INVALID_ARG: return "invalid argument";
+    case FF_ERR_WORKSPACE: return "workspace missing, too small or misaligned";
+    case FF_ERR_NO_TREE: return "no tree: call ff_build_tree first";
+    case FF_ERR_CAPACITY: return "cell pool capacity exceeded";
+    case FF_ERR_CUDA: return "CUDA error (see ff_last_error)";
+    default: return "unknown error code";
+    }
+}
+
+extern "C" const char* ff_last_error(ff_ctx* c) { return c ? c->last_error : ""; }

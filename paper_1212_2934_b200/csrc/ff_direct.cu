@@ -1,0 +1,166 @@
+// ff_direct.cu -- a8 tiled all-pairs field + force, and the FP32 FMA-pipe microbenchmark.
+//
+// Paper: Algorithm 1: one thread per target k, sources staged
+// through shared memory in tiles of blockDim.x, self excluded by index (line 5).
+// Kept from that design: the tiling and the one-thread-one-target mapping.
+// Changed: the self test runs only in the one tile that can contain k (block
+// uniform branch); each tile's fp32 partial sums are folded into fp64 running
+// sums so that 10^6 sources keep 1e-5 relative accuracy; small N is split over
+// source chunks so the grid still covers all 148 SMs.
+#include "ff_internal.cuh"
+
+__device__ __forceinline__ void ff_pair_accum_d(float dx, float dy, float dz, float rinv, float ux, float uy, float uz,
+                                                float mx, float my, float mz, float& hx, float& hy, float& hz,
+                                                float& fx, float& fy, float& fz, float& sk)
+{
+    float rinv2 = rinv * rinv;
+    float rinv3 = rinv2 * rinv;
+    float r5x3 = 3.0f * (rinv3 * rinv2);
+    float a = fmaf(mz, dz, fmaf(my, dy, mx * dx));
+    float b = fmaf(uz, dz, fmaf(uy, dy, ux * dx));
+    float cc = fmaf(mz, uz, fmaf(my, uy, mx * ux));
+    float ca = a * r5x3;
+    float cb = b * r5x3;
+    hx = fmaf(ca, dx, hx); hy = fmaf(ca, dy, hy); hz = fmaf(ca, dz, hz);
+    hx = fmaf(-rinv3, mx, hx); hy = fmaf(-rinv3, my, hy); hz = fmaf(-rinv3, mz, hz);
+    float t = (a * b) * rinv2;
+    float cr = fmaf(-5.0f, t, cc) * r5x3;
+    fx = fmaf(cr, dx, fx); fy = fmaf(cr, dy, fy); fz = fmaf(cr, dz, fz);
+    fx = fmaf(cb, mx, fx); fy = fmaf(cb, my, fy); fz = fmaf(cb, mz, fz);
+    sk += ca;
+}
+
+// rsqrt with one Newton step: the all-pairs tolerance is 1e-5 on sums dominated by a few near terms
+__device__ __forceinline__ float ff_rsqrt_nr(float r2)
+{
+    float y = rsqrtf(r2);
+    return y * fmaf(-0.5f * r2, y * y, 1.5f);
+}
+
+// grid = (target blocks, source splits).  Block (bx, by) accumulates, for its 256 targets, the
+// sources of tiles by, by + splits, by + 2 splits, ...
+__global__ void __launch_bounds__(FF_DIRECT_THREADS)
+ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n, int splits,
+            double* __restrict__ part, float* __restrict__ H_out, float* __restrict__ F_out)
+{
+    __shared__ float4 spos[FF_DIRECT_THREADS], smom[FF_DIRECT_THREADS];
+    const int t = threadIdx.x;
+    const int k = blockIdx.x * FF_DIRECT_THREADS + t;
+    const int kk = min(k, n - 1);
+    const float px = __ldg(pos + 3 * (size_t)kk), py = __ldg(pos + 3 * (size_t)kk + 1), pz = __ldg(pos + 3 * (size_t)kk + 2);
+    const float ux = __ldg(mom + 3 * (size_t)kk), uy = __ldg(mom + 3 * (size_t)kk + 1), uz = __ldg(mom + 3 * (size_t)kk + 2);
+    double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };
+    const int n_tiles = (n + FF_DIRECT_THREADS - 1) / FF_DIRECT_THREADS;
+    for (int tile = blockIdx.y; tile < n_tiles; tile += splits) {
+        int j = tile * FF_DIRECT_THREADS + t;
+        float4 sp = make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.f), sv = make_float4(0.f, 0.f, 0.f, 0.f);   // padding: zero moment, far away
+        if (j < n) {
+            sp = make_float4(__ldg(pos + 3 * (size_t)j), __ldg(pos + 3 * (size_t)j + 1), __ldg(pos + 3 * (size_t)j + 2), 0.f);
+            sv = make_float4(__ldg(mom + 3 * (size_t)j), __ldg(mom + 3 * (size_t)j + 1), __ldg(mom + 3 * (size_t)j + 2), 0.f);
+        }
+        __syncthreads();
+        spos[t] = sp; smom[t] = sv;
+        __syncthreads();
+        float hx = 0.f, hy = 0.f, hz = 0.f, fx = 0.f, fy = 0.f, fz = 0.f, sk = 0.f;
+        if (tile == blockIdx.x) {            // the only tile that holds this block's own targets
+#pragma unroll 4
+            for (int i = 0; i < FF_DIRECT_THREADS; ++i) {
+                float4 a = spos[i], m = smom[i];
+                float dx = px - a.x, dy = py - a.y, dz = pz - a.z;
+                float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                float rinv = (i == t) ? 0.0f : ff_rsqrt_nr(r2);   // j + i != k (Alg. 1 line 5)
+                ff_pair_accum_d(dx, dy, dz, rinv, ux, uy, uz, m.x, m.y, m.z, hx, hy, hz, fx, fy, fz, sk);
+            }
+        } else {
+#pragma unroll 8
+            for (int i = 0; i < FF_DIRECT_THREADS; ++i) {
+                float4 a = spos[i], m = smom[i];
+                float dx = px - a.x, dy = py - a.y, dz = pz - a.z;
+                float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                ff_pair_accum_d(dx, dy, dz, ff_rsqrt_nr(r2), ux, uy, uz, m.x, m.y, m.z, hx, hy, hz, fx, fy, fz, sk);
+            }
+        }
+        acc[0] += hx; acc[1] += hy; acc[2] += hz; acc[3] += fx; acc[4] += fy; acc[5] += fz; acc[6] += sk;
+    }
+    if (k >= n) return;
+    acc[3] += acc[6] * (double)ux; acc[4] += acc[6] * (double)uy; acc[5] += acc[6] * (double)uz;
+    if (splits == 1) {
+        if (H_out) { H_out[3 * (size_t)k] = (float)acc[0]; H_out[3 * (size_t)k + 1] = (float)acc[1]; H_out[3 * (size_t)k + 2] = (float)acc[2]; }
+        if (F_out) { F_out[3 * (size_t)k] = (float)acc[3]; F_out[3 * (size_t)k + 1] = (float)acc[4]; F_out[3 * (size_t)k + 2] = (float)acc[5]; }
+    } else {
+        double* p = part + ((size_t)blockIdx.y * n + k) * 6;
+#pragma unroll
+        for (int a = 0; a < 6; ++a) p[a] = acc[a];
+    }
+}
+
+__global__ void __launch_bounds__(256)
+ff_k_direct_reduce(const double* __restrict__ part, int n, int splits, float* __restrict__ H_out, float* __restrict__ F_out)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    double acc[6] = { 0, 0, 0, 0, 0, 0 };
+    for (int s = 0; s < splits; ++s) {
+        const double* p = part + ((size_t)s * n + k) * 6;
+#pragma unroll
+        for (int a = 0; a < 6; ++a) acc[a] += p[a];
+    }
+    if (H_out) { H_out[3 * (size_t)k] = (float)acc[0]; H_out[3 * (size_t)k + 1] = (float)acc[1]; H_out[3 * (size_t)k + 2] = (float)acc[2]; }
+    if (F_out) { F_out[3 * (size_t)k] = (float)acc[3]; F_out[3 * (size_t)k + 1] = (float)acc[4]; F_out[3 * (size_t)k + 2] = (float)acc[5]; }
+}
+
+int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n64, float* H_out, float* F_out)
+{
+    int n = (int)n64;
+    int tblocks = (n + FF_DIRECT_THREADS - 1) / FF_DIRECT_THREADS;
+    // enough blocks for ~4 per SM; the partial-sum scratch bounds targets * splits
+    int want = c->num_sms * 4;
+    int splits = (want + tblocks - 1) / tblocks;
+    if (splits > tblocks) splits = tblocks;
+    while (splits > 1 && (int64_t)splits * n > FF_DIRECT_SPLIT_ELEMS) --splits;
+    if (splits < 1) splits = 1;
+    dim3 grid(tblocks, splits);
+    FF_LAUNCH(c, ff_k_direct, grid, FF_DIRECT_THREADS, 0, pos, mom, n, splits, c->direct_part, H_out, F_out);
+    if (splits > 1)
+        FF_LAUNCH(c, ff_k_direct_reduce, (n + 255) / 256, 256, 0, c->direct_part, n, splits, H_out, F_out);
+    return FF_OK;
+}
+
+// ---- FP32 FMA-pipe peak: 8 independent dependent chains per thread ---------------------
+__global__ void __launch_bounds__(256) ff_k_fma_peak(int iters, float seed, float* __restrict__ sink)
+{
+    float x0 = seed + threadIdx.x, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f, x4 = x0 + 4.f, x5 = x0 + 5.f,
+          x6 = x0 + 6.f, x7 = x0 + 7.f;
+    const float a = 0.999f + seed * 1e-9f, b = 1e-3f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            x0 = fmaf(x0, a, b); x1 = fmaf(x1, a, b); x2 = fmaf(x2, a, b); x3 = fmaf(x3, a, b);
+            x4 = fmaf(x4, a, b); x5 = fmaf(x5, a, b); x6 = fmaf(x6, a, b); x7 = fmaf(x7, a, b);
+        }
+    }
+    float s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 12345.678f) sink[0] = s;          // never true in practice; keeps the chains alive
+}
+
+int ff_launch_fp32_peak(ff_ctx* c, int iters, double* tflops)
+{
+    if (iters < 1) iters = 1;
+    int blocks = c->num_sms * 8;
+    cudaEvent_t e0, e1;
+    FF_CUDA(c, cudaEventCreate(&e0));
+    FF_CUDA(c, cudaEventCreate(&e1));
+    float* sink = reinterpret_cast<float*>(c->direct_part);
+    FF_LAUNCH(c, ff_k_fma_peak, blocks, 256, 0, iters, 1.0f, sink);     // warm-up
+    FF_CUDA(c, cudaEventRecord(e0, c->stream));
+    FF_LAUNCH(c, ff_k_fma_peak, blocks, 256, 0, iters, 1.0f, sink);
+    FF_CUDA(c, cudaEventRecord(e1, c->stream));
+    FF_CUDA(c, cudaEventSynchronize(e1));
+    float ms = 0.f;
+    FF_CUDA(c, cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    double flop = 2.0 * 64.0 * (double)iters * 256.0 * (double)blocks;
+    *tflops = flop / ((double)ms * 1e-3) / 1e12;
+    return FF_OK;
+}

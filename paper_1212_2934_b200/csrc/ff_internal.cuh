@@ -1,0 +1,146 @@
+// ff_internal.cuh -- context layout and launch helpers shared by the .cu files of libff.
+// Nothing here is visible through include/ff.h.  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/ff.h"
+
+#define FF_WARP 32
+#define FF_FULL 0xffffffffu
+
+// ---- radix sort geometry (ff_sort.cu) --------------------------------------
+#define FF_SORT_THREADS 256
+#define FF_SORT_ROUNDS 8                                   // keys per thread
+#define FF_SORT_TILE (FF_SORT_THREADS * FF_SORT_ROUNDS)    // keys per block
+#define FF_RADIX_BITS 8
+#define FF_RADIX 256
+
+// ---- scan geometry (ff_build.cu) --------------------------------------------
+#define FF_SCAN_THREADS 256
+#define FF_SCAN_ITEMS 8
+#define FF_SCAN_TILE (FF_SCAN_THREADS * FF_SCAN_ITEMS)
+
+// ---- walk geometry (ff_walk.cu) ---------------------------------------------
+#define FF_WALK_WARPS 8            // warps (= target groups) per block
+#define FF_WALK_STACK 1024         // traversal stack entries per warp
+#define FF_WALK_PEND 64            // pending interaction ring per warp (two batches of 32)
+
+// ---- direct geometry (ff_direct.cu) -------------------------------------------
+#define FF_DIRECT_THREADS 256
+#define FF_DIRECT_SPLIT_ELEMS (1 << 19)   // max targets*splits whose partial sums fit the scratch
+
+// Small block of device-resident scalars: written and read by kernels only, so
+// that build/eval never needs a host read (SURVEY.md 8(b) "no host round-trip").
+struct ff_globals {
+    uint32_t bbox_ord[8];     // ordered-uint encoding of min xyz [0..2] and max xyz [4..6]
+    float lo[3];              // root cube origin
+    float S;                  // root cube side
+    float inv;                // fl(1024 / S)
+    int32_t n_cells;          // internal cells of the current tree
+    int32_t error;            // sticky device-side error flag (FF_ERR_*)
+    int32_t pad0;
+    unsigned long long counters[3];   // n_cell, n_particle, n_mac (FF_OPT_COUNTERS)
+    uint32_t digit_total[FF_RADIX];   // per-pass digit totals (ff_sort.cu)
+};
+
+struct ff_ctx {
+    int64_t N;                // capacity
+    int64_t n;                // particles of the current tree / call
+    int64_t cell_cap;         // capacity of the cell pool
+    float theta;
+    int nleaf;
+    int count_enabled;
+    int timing_enabled;
+    int tree_built;
+    int moments_valid;
+    int device;
+    int num_sms;
+    cudaStream_t stream;
+    uint64_t launches;
+    char last_error[256];
+
+    // workspace carve-up (device pointers)
+    char* ws; size_t ws_bytes;
+    ff_globals* g;
+    uint32_t *key[2], *idx[2];        // ping-pong buffers of the sort; result in [0]
+    float4 *pos_s, *mom_s;            // sorted particles
+    int32_t* leaf_count;              // [N]
+    int32_t* cell_base;               // [N] exclusive scan of cells starting at each slot
+    uint32_t* scan_blk;               // block sums of the scan
+    uint32_t* sort_hist;              // [FF_RADIX][n_tiles]
+    int32_t *cell_first, *cell_end, *cell_level;
+    int32_t* cell_child;              // [cap][8]
+    float4 *cell_centre, *cell_moment;
+    double *cell_sum_u, *cell_sum_p;  // [cap][3] fp64 sums in the fixed order
+    double* direct_part;              // partial sums of the split direct kernel
+    float *stage_pos, *stage_mom, *stage_H, *stage_F;   // device staging of the *_host calls / ff_step fields
+    float* step_fsr;                  // [N][3] short-range force (ff_step)
+
+    cudaEvent_t ev[FF_N_PHASES][2];
+    int ev_valid[FF_N_PHASES];
+};
+
+// ---- error plumbing ------------------------------------------------------------
+static inline int ff_cuda_fail(ff_ctx* c, cudaError_t e, const char* what)
+{
+    if (c) snprintf(c->last_error, sizeof(c->last_error), "%s: %s", what, cudaGetErrorString(e));
+    return FF_ERR_CUDA;
+}
+
+#define FF_CUDA(c, call)                                            \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) return ff_cuda_fail((c), e__, #call); \
+    } while (0)
+
+// launch + count + check
+#define FF_LAUNCH(c, kernel, grid, block, smem, ...)                          \
+    do {                                                                      \
+        kernel<<<(grid), (block), (smem), (c)->stream>>>(__VA_ARGS__);        \
+        (c)->launches++;                                                      \
+        cudaError_t e__ = cudaGetLastError();                                 \
+        if (e__ != cudaSuccess) return ff_cuda_fail((c), e__, #kernel);       \
+    } while (0)
+
+static inline void ff_phase_begin(ff_ctx* c, int ph)
+{
+    if (c->timing_enabled) cudaEventRecord(c->ev[ph][0], c->stream);
+}
+static inline void ff_phase_end(ff_ctx* c, int ph)
+{
+    if (c->timing_enabled) { cudaEventRecord(c->ev[ph][1], c->stream); c->ev_valid[ph] = 1; }
+}
+
+// ---- phase launchers implemented in the other .cu files -------------------------
+int ff_launch_bbox_keys(ff_ctx* c, const float* pos);
+int ff_launch_sort(ff_ctx* c, const float* pos);
+int ff_launch_build(ff_ctx* c);
+int ff_launch_gather_mom(ff_ctx* c, const float* mom);
+int ff_launch_moments(ff_ctx* c);
+int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out);
+int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n, float* H_out, float* F_out);
+int ff_launch_fp32_peak(ff_ctx* c, int iters, double* tflops);
+int ff_launch_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n,
+                   const ff_step_params* p, uint64_t step_index);
+
+// ---- small device helpers --------------------------------------------------------
+__device__ __forceinline__ uint32_t ff_f2ord(float f)
+{
+    uint32_t u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float ff_ord2f(uint32_t o)
+{
+    return __uint_as_float((o & 0x80000000u) ? (o & 0x7fffffffu) : ~o);
+}
+__device__ __forceinline__ int ff_lane() { return threadIdx.x & 31; }
+
+// number of leading octant digits two 30-bit keys share (10 if equal)
+__device__ __forceinline__ int ff_common_levels(uint32_t a, uint32_t b)
+{
+    uint32_t x = a ^ b;
+    return x ? (__clz(x) - 2) / 3 : FF_MAX_LEVEL;
+}

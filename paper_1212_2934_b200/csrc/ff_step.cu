@@ -1,0 +1,171 @@
+// ff_step.cu -- the steps either side of the hot path: Lennard-Jones
+// short-range force (Eq. 13) and the Euler-Maruyama update
+// of the reduced equations of motion Eq. 7-9, i.e. the second half of
+// the paper's kernel 5 and its kernel 6.
+//
+// Rotation is integrated in the vector form of DESIGN.md (reading Q12):
+//   d(omega)/dtau = 5/2 (u x h - Gamma_r omega) + noise,   du/dtau = omega x u,  |u| = 1
+// which is Eq. 7-8 (2/5 = I / (M R^2)) without the polar-angle singularity.
+#include "ff_internal.cuh"
+
+#define FF_LJ_MAX_LEVEL 7                       // cell table of at most 8^7 cells
+
+__device__ __forceinline__ uint32_t ff_compact10(uint32_t v)    // inverse of the 3-way bit spread
+{
+    v &= 0x09249249u;
+    v = (v | (v >> 2)) & 0x030C30C3u;
+    v = (v | (v >> 4)) & 0x0300F00Fu;
+    v = (v | (v >> 8)) & 0x030000FFu;
+    v = (v | (v >> 16)) & 0x000003FFu;
+    return v;
+}
+__device__ __forceinline__ uint32_t ff_spread10s(uint32_t v)
+{
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+
+// deepest level (<= FF_LJ_MAX_LEVEL) whose cell side S 2^-l is still >= the cut-off: computed on the
+// device from the device-resident root cube so that ff_step needs no host read
+__device__ __forceinline__ int ff_lj_level(float S, float rc)
+{
+    int lev = 0;
+    while (lev < FF_LJ_MAX_LEVEL && ldexpf(S, -(lev + 1)) >= rc) ++lev;
+    return lev;
+}
+
+// cell table over the level-`lev` cells of the sorted keys: [start, end) per cell prefix
+__global__ void __launch_bounds__(256) ff_k_cell_table(const uint32_t* __restrict__ key, int n,
+                                                       const ff_globals* __restrict__ g, float rc,
+                                                       int32_t* __restrict__ start, int32_t* __restrict__ end)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int lev = ff_lj_level(g->S, rc);
+    int sh = 3 * (FF_MAX_LEVEL - lev);
+    uint32_t c = __ldg(key + i) >> sh;
+    if (i == 0 || (__ldg(key + i - 1) >> sh) != c) start[c] = i;
+    if (i == n - 1 || (__ldg(key + i + 1) >> sh) != c) end[c] = i + 1;
+}
+
+// Eq. 13: f_k^sr = 24 eps sum_j rho_kj / rho_kj^2 [ (sigma/rho_kj)^12 - (sigma/rho_kj)^6 ], pairs within rc
+__global__ void __launch_bounds__(128)
+ff_k_lj(const uint32_t* __restrict__ key, const float4* __restrict__ pos_s, const uint32_t* __restrict__ perm, int n,
+        const ff_globals* __restrict__ g, const int32_t* __restrict__ start, const int32_t* __restrict__ end, float eps,
+        float sigma, float rc, float* __restrict__ fsr)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    int lev = ff_lj_level(g->S, rc);
+    float4 p = pos_s[s];
+    uint32_t c = __ldg(key + s) >> (3 * (FF_MAX_LEVEL - lev));
+    int qx = (int)ff_compact10(c >> 2), qy = (int)ff_compact10(c >> 1), qz = (int)ff_compact10(c);
+    int side = 1 << lev;
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    float rc2 = rc * rc, s2 = sigma * sigma;
+    for (int dx = -1; dx <= 1; ++dx)
+        for (int dy = -1; dy <= 1; ++dy)
+            for (int dz = -1; dz <= 1; ++dz) {
+                int x = qx + dx, y = qy + dy, z = qz + dz;
+                if (x < 0 || y < 0 || z < 0 || x >= side || y >= side || z >= side) continue;
+                uint32_t cc = (ff_spread10s((uint32_t)x) << 2) | (ff_spread10s((uint32_t)y) << 1) | ff_spread10s((uint32_t)z);
+                int b = __ldg(start + cc), e = __ldg(end + cc);
+                for (int j = b; j < e; ++j) {
+                    if (j == s) continue;
+                    float4 q = __ldg(pos_s + j);
+                    float rx = p.x - q.x, ry = p.y - q.y, rz = p.z - q.z;
+                    float r2 = fmaf(rz, rz, fmaf(ry, ry, rx * rx));
+                    if (r2 < rc2) {
+                        float ir2 = 1.0f / r2;
+                        float sr2 = s2 * ir2, sr6 = sr2 * sr2 * sr2;
+                        float w = 24.0f * eps * ir2 * (sr6 * sr6 - sr6);
+                        fx = fmaf(w, rx, fx); fy = fmaf(w, ry, fy); fz = fmaf(w, rz, fz);
+                    }
+                }
+            }
+    size_t o = (size_t)__ldg(perm + s) * 3;
+    fsr[o] = fx; fsr[o + 1] = fy; fsr[o + 2] = fz;
+}
+
+// counter-based unit Gaussians: splitmix64 finaliser -> Box-Muller
+__device__ __forceinline__ uint64_t ff_mix64(uint64_t z)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+__device__ __forceinline__ void ff_gauss2(uint64_t seed, uint64_t step, uint64_t k, uint32_t lane, float& g0, float& g1)
+{
+    uint64_t z = ff_mix64(seed * 0x9E3779B97F4A7C15ull + step);
+    z = ff_mix64(z ^ (k * 0xD1B54A32D192ED03ull + lane));
+    float u1 = ((float)(uint32_t)(z >> 40) + 0.5f) * (1.0f / 16777216.0f);
+    float u2 = ((float)(uint32_t)((z >> 8) & 0xffffffu)) * (1.0f / 16777216.0f);
+    float r = sqrtf(-2.0f * __logf(u1));
+    __sincosf(6.28318530718f * u2, &g1, &g0);
+    g0 *= r; g1 *= r;
+}
+
+__global__ void __launch_bounds__(256)
+ff_k_integrate(int n, float* __restrict__ pos, float* __restrict__ vel, float* __restrict__ mom,
+               float* __restrict__ angvel, const float* __restrict__ H, const float* __restrict__ F,
+               const float* __restrict__ fsr, ff_step_params p, uint64_t step)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    size_t o = 3 * (size_t)k;
+    float x[3], v[3], u[3], w[3], h[3], f[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        x[a] = pos[o + a]; v[a] = vel[o + a]; u[a] = mom[o + a]; w[a] = angvel[o + a];
+        h[a] = H[o + a] + p.h_ext[a];
+        f[a] = F[o + a] + (fsr ? fsr[o + a] : 0.0f);
+    }
+    float xi[6] = { 0.f, 0.f, 0.f, 0.f, 0.f, 0.f };
+    if (p.noise_d != 0.0f || p.noise_r != 0.0f) {
+        ff_gauss2(p.seed, step, (uint64_t)k, 0u, xi[0], xi[1]);
+        ff_gauss2(p.seed, step, (uint64_t)k, 1u, xi[2], xi[3]);
+        ff_gauss2(p.seed, step, (uint64_t)k, 2u, xi[4], xi[5]);
+    }
+    float sq = sqrtf(p.dtau);
+    // torque u x h
+    float t[3] = { u[1] * h[2] - u[2] * h[1], u[2] * h[0] - u[0] * h[2], u[0] * h[1] - u[1] * h[0] };
+    // omega x u with the OLD omega (explicit Euler-Maruyama)
+    float du[3] = { w[1] * u[2] - w[2] * u[1], w[2] * u[0] - w[0] * u[2], w[0] * u[1] - w[1] * u[0] };
+    float un[3], nn = 0.f;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        float xn = x[a] + p.dtau * v[a];
+        float vn = v[a] + p.dtau * (f[a] - p.gamma_d * v[a]) + p.noise_d * sq * xi[a];
+        float wn = w[a] + p.dtau * 2.5f * (t[a] - p.gamma_r * w[a]) + p.noise_r * sq * xi[3 + a];
+        un[a] = u[a] + p.dtau * du[a];
+        nn += un[a] * un[a];
+        pos[o + a] = xn; vel[o + a] = vn; angvel[o + a] = wn;
+    }
+    float inv = rsqrtf(nn);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) mom[o + a] = un[a] * inv;
+}
+
+int ff_launch_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n64,
+                   const ff_step_params* p, uint64_t step_index)
+{
+    int n = (int)n64;
+    const float* fsr = nullptr;
+    if (p->lj_epsilon != 0.0f) {
+        if (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f)) return FF_ERR_INVALID_ARG;
+        size_t cells = (size_t)1 << (3 * FF_LJ_MAX_LEVEL);                   // table sized for the deepest level
+        int32_t* start = reinterpret_cast<int32_t*>(c->direct_part);       // 2 * 8^7 * 4 B = 16 MB <= scratch
+        int32_t* end = start + cells;
+        FF_CUDA(c, cudaMemsetAsync(start, 0, 2 * cells * sizeof(int32_t), c->stream));
+        FF_LAUNCH(c, ff_k_cell_table, (n + 255) / 256, 256, 0, c->key[0], n, c->g, p->lj_cutoff, start, end);
+        FF_LAUNCH(c, ff_k_lj, (n + 127) / 128, 128, 0, c->key[0], c->pos_s, c->idx[0], n, c->g, start, end,
+                  p->lj_epsilon, p->lj_sigma, p->lj_cutoff, c->step_fsr);
+        fsr = c->step_fsr;
+    }
+    FF_LAUNCH(c, ff_k_integrate, (n + 255) / 256, 256, 0, n, pos, vel, mom, angvel, c->stage_H, c->stage_F, fsr, *p,
+              step_index);
+    return FF_OK;
+}
