@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement of BASELINE.json:
+
+    dipole field+force particle-evals/s & ms/step at N = 2^20, theta = 0.5; FP32-pipe % of peak
+
+One "step" = one pass of the whole hot path: ff_build_tree
+(bounding box, Morton keys, radix sort, octree) + ff_eval_bh (cell moments, tree walk, scatter to
+caller order) on config 3 (1 048 576 hard-sphere dipoles, volume fraction 0.1, isotropic moments),
+inputs resident in HBM.  Prints ONE JSON line (see the driver contract in the task statement).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n N] [--quick]
+
+N > 1: launched under torchrun, one rank per GPU; every rank runs an independent replica of the
+workload with its own seed (the paper averages over independent realisations), no
+data-path collective, "scaling": "weak".
+--impl reference: the fp64 oracle (oracle/), as it stands, on the host cores of this box.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "dipole field+force particle-evals/s (Barnes-Hut step: sort+build+moments+walk), N=2^20, theta=0.5"
+UNIT = "particle-evals/s"
+FLOP_PER_INTERACTION = 60.0      # 21 FFMA x2 + 17 FADD/FMUL + 1 MUFU.RSQ per h+f pair term
+FP32_LANES_PER_SM = 128
+# dram__bytes_read.sum + dram__bytes_write.sum of one ff_k_walk launch at config 3, from the
+# `ncu --set full` capture summarised in profiles/ (None until a capture exists)
+WALK_DRAM_TRAFFIC_BYTES = None
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                if t0 - 0.05 <= ts <= t1 + 0.15:
+                    sm.append(float(f[0]))
+                    mx.append(float(f[1]))
+                    for nm, v in zip(names, f[3:7]):
+                        if v.lower().startswith("active"):
+                            reasons.add(nm)
+            except ValueError:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _workload(n, seed):
+    import ffgen
+    c = ffgen.config(3, seed=seed, N=n)
+    return c
+
+
+def _oracle_step(c, groups, nthreads=0):
+    """One oracle pass on a bounded sample: full tree + moments, walk of `groups` only.
+    Returns (t_build, t_moments, t_walk)."""
+    import oracle
+    t0 = time.perf_counter()
+    t = oracle.Tree(c["pos"])
+    t1 = time.perf_counter()
+    t.moments(c["mom"])
+    t2 = time.perf_counter()
+    t.eval(c["theta"], 32, groups=groups, nthreads=nthreads)
+    t3 = time.perf_counter()
+    return t1 - t0, t2 - t1, t3 - t2
+
+
+def _oracle_rate(c, n_groups_sample, nthreads=0):
+    """Extrapolated whole-job particle-evals/s of the oracle from a bounded sample."""
+    N = c["N"]
+    n_groups = (N + 31) // 32
+    groups = np.random.default_rng(0).choice(n_groups, min(n_groups_sample, n_groups), replace=False)
+    tb, tm, tw = _oracle_step(c, groups, nthreads)
+    full = tb + tm + tw * n_groups / len(groups)
+    return N / full, dict(t_build_s=tb, t_moments_s=tm, t_walk_sample_s=tw, groups=int(len(groups)))
+
+
+def run_reference(args):
+    import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    c = _workload(args.n, 0)
+    cores = oracle.max_threads()
+    n_groups = (c["N"] + 31) // 32
+    sample = min(n_groups, 1024)
+    for _ in range(args.warmup):
+        _oracle_rate(c, sample)
+    t0 = time.perf_counter()
+    rates = [_oracle_rate(c, sample)[0] for _ in range(args.steps)]
+    wall = time.perf_counter() - t0
+    value = float(np.mean(rates))
+    desc = ("fp64 oracle (oracle/ff_oracle.c), per step: full tree build + cell moments over all N, walk of %d sampled "
+            "groups of 32 targets, walk time extrapolated to all %d groups" % (sample, n_groups))
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * c["N"] / value, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config 3 of BASELINE.json: N=%d hard-sphere dipoles, phi=0.1, isotropic moments, theta=0.5, "
+                               "group rule W=32" % c["N"], "N": c["N"], "theta": c["theta"]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "wall_s": wall,
+    }
+    print(json.dumps(out))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1212_2934_b200 as ff
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    c = _workload(args.n, rank)                       # independent replica per rank
+    N, theta = c["N"], c["theta"]
+    pos_h = torch.from_numpy(c["pos"]).pin_memory()
+    mom_h = torch.from_numpy(c["mom"]).pin_memory()
+    pos, mom = pos_h.to(dev), mom_h.to(dev)
+    H, F = torch.empty_like(pos), torch.empty_like(pos)
+    ctx = ff.FFContext(N, theta, device=dev, timing=True)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def step():
+        ctx.build_tree(pos)
+        ctx.eval_bh(pos, mom, H, F)
+
+    # interaction counts of this workload (separate, untimed run of the counting kernel variant)
+    ctx.set_option(ff.FF_OPT_COUNTERS, 1)
+    step()
+    n_cell, n_part, n_mac = ctx.counters()
+    ctx.set_option(ff.FF_OPT_COUNTERS, 0)
+    interactions = n_cell + n_part
+
+    for _ in range(max(args.warmup, 3)):
+        flush.zero_()
+        step()
+    torch.cuda.synchronize()
+    ctx.timings()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    phases = {k: 0.0 for k in ff.PHASES}
+    l0 = ctx.launch_count()
+    t_wall0 = time.time()
+    for i in range(args.steps):
+        flush.zero_()                                  # evict the previous step from L2 (not timed)
+        ev[i][0].record()
+        step()
+        ev[i][1].record()
+        ev[i][1].synchronize()
+        for k, v in ctx.timings().items():
+            phases[k] += v
+    torch.cuda.synchronize()
+    t_wall1 = time.time()
+    launches = ctx.launch_count() - l0
+    if world > 1:
+        dist.barrier()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    tt = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    total_ms = float(tt.item())
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    ms_per_step = total_ms / args.steps
+    value = world * N / (ms_per_step * 1e-3)
+    phases = {k: v / args.steps for k, v in phases.items()}
+
+    # ---- end to end through the C ABI with host buffers (H2D + step + D2H inside the timed region)
+    H_h = torch.empty((N, 3), dtype=torch.float32).pin_memory()
+    F_h = torch.empty((N, 3), dtype=torch.float32).pin_memory()
+    for _ in range(2):
+        ctx.eval_bh_host(pos_h, mom_h, H_h, F_h)
+    e2e_steps = max(3, min(args.steps, 10))
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2e_ms = 0.0
+    for _ in range(e2e_steps):
+        flush.zero_()
+        e0.record()
+        ctx.eval_bh_host(pos_h, mom_h, H_h, F_h)
+        e1.record()
+        e1.synchronize()
+        e2e_ms += e0.elapsed_time(e1)
+    te = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * N / (float(te.item()) / e2e_steps * 1e-3)
+    checksum = float(H_h.double().abs().sum() + F_h.double().abs().sum())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the walk): plain FP32 ALU work
+    peaks, peak_src = _peaks()
+    sm_max = float(clocks["sm_max_mhz"] or peaks.get("sm_max_mhz", 1965.0))
+    num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_tflops = num_sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    walk_ms = phases["walk"]
+    achieved = interactions * FLOP_PER_INTERACTION / (walk_ms * 1e-3) / 1e12
+    fma_peak = ctx.measure_fp32_peak(1 << 14)
+    roofline = {
+        "bound": "alu", "kernel": "ff_k_walk", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved / peak_tflops, "traffic": WALK_DRAM_TRAFFIC_BYTES,
+        "peak_source": "nominal: %d SMs x 128 FP32 lanes x 2 flop x %.0f MHz (clocks.max.sm); MEASURED_PEAKS.json (%s) "
+                       "holds no FP32 figure" % (num_sms, sm_max, peak_src),
+        "measured_fma_peak_tflops": fma_peak, "frac_of_measured_fma": achieved / fma_peak,
+        "interactions_per_launch": interactions, "flop_per_interaction": FLOP_PER_INTERACTION,
+        "kernel_ms": walk_ms, "kernel_share_of_step": walk_ms / ms_per_step,
+        "interactions_per_s": interactions / (walk_ms * 1e-3),
+    }
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    # algorithmic bytes per particle of the HBM-bound phases (DESIGN.md / SURVEY.md 8(d))
+    alg_bytes = {"bbox_keys": 12 + 12 + 4, "sort": 4 * (4 + 16) + 4 + 12 + 16, "build": 26, "moments": 12 + 16 + 122}
+    hbm_phases = {k: {"ms": phases[k], "achieved_gbs": alg_bytes[k] * N / (phases[k] * 1e-3) / 1e9,
+                      "frac_of_hbm_peak": alg_bytes[k] * N / (phases[k] * 1e-3) / 1e9 / hbm}
+                  for k in alg_bytes if phases[k] > 0}
+
+    extras = {}
+    if not args.quick:
+        # GPU direct all-pairs on the same workload (a8), once; and the BH-vs-all-pairs error vs theta
+        torch.cuda.synchronize()
+        ctx.timings()
+        Hd, Fd = ctx.eval_direct(pos, mom)
+        torch.cuda.synchronize()
+        d_ms = ctx.timings()["direct"]
+        pairs = float(N) * (N - 1)
+        extras["gpu_direct"] = {"ms": d_ms, "pair_interactions_per_s": pairs / (d_ms * 1e-3),
+                                "tflops": pairs * 64.0 / (d_ms * 1e-3) / 1e12,
+                                "frac_of_fp32_peak": pairs * 64.0 / (d_ms * 1e-3) / 1e12 / peak_tflops,
+                                "flop_per_pair": 64.0, "speedup_bh_over_direct": d_ms / ms_per_step}
+        errs = {}
+        for th in (0.3, 0.5, 0.7):
+            ctx.set_option(ff.FF_OPT_THETA, th)
+            Hb, Fb = ctx.eval_bh(pos, mom)
+            errs[str(th)] = {"H_rel_l2": float((Hb - Hd).double().norm() / Hd.double().norm()),
+                             "F_rel_l2": float((Fb - Fd).double().norm() / Fd.double().norm())}
+        ctx.set_option(ff.FF_OPT_THETA, theta)
+        extras["bh_vs_allpairs_error"] = {"reference": "GPU direct kernel (ff_eval_direct)", "by_theta": errs}
+
+    # ---- the oracle timed beside it on this box's host cores (bounded sample)
+    import oracle
+    cores = oracle.max_threads()
+    sample = 2048 if N >= (1 << 20) else max(1, min(2048, (N + 31) // 32))
+    cpu_value, cpu_detail = _oracle_rate(c, sample)
+    cpu_1, _ = _oracle_rate(c, max(1, sample // 8), nthreads=1)
+    cpu_baseline = {"value": cpu_value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                    "sample": "full tree + moments over all N, walk of %d sampled groups (%d targets) extrapolated to all "
+                              "groups" % (cpu_detail["groups"], cpu_detail["groups"] * 32),
+                    "detail": cpu_detail, "single_thread_value": cpu_1}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "config 3 of BASELINE.json: N=%d hard-sphere dipoles (d=1), phi=0.1, isotropic unit moments, "
+                               "theta=0.5, tree rebuilt every step, H and F" % N,
+                   "N": N, "theta": theta, "group": 32, "nleaf": 1, "l2": "flushed between timed steps (512 MB memset)",
+                   "replicas": world},
+        "clocks": clocks, "gpu_launches": int(launches), "launches_per_step": launches / args.steps,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 12, "d2h_bytes_per_step": 2 * N * 12,
+                "steps": e2e_steps, "api": "ff_eval_bh_host (pinned host buffers)", "checksum": checksum},
+        "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "phases_ms": phases, "hbm_phases": hbm_phases,
+        "counters": {"n_cell": n_cell, "n_particle": n_part, "n_mac_tests": n_mac,
+                     "interactions_per_target": interactions / N},
+        "step_ms_min_max": [min(step_ms), max(step_ms)],
+    }
+    out.update(extras)
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=1 << 20, help="particles (default: config 3, 2^20)")
+    ap.add_argument("--quick", action="store_true", help="skip the direct kernel and the theta sweep")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

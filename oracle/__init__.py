@@ -42,7 +42,7 @@ def _load():
         lib.ffo_pair.argtypes = [vp] * 6
         lib.ffo_max_threads.restype = i32
         lib.ffo_allpairs.restype = i32
-        lib.ffo_allpairs.argtypes = [i64, vp, vp, i64, vp, vp, vp, i32]
+        lib.ffo_allpairs.argtypes = [i64, vp, vp, i64, vp, vp, vp, vp, i32]
         lib.ffo_tree_build.restype = vp
         lib.ffo_tree_build.argtypes = [i64, vp, i32]
         lib.ffo_tree_free.restype = None
@@ -60,7 +60,7 @@ def _load():
         lib.ffo_tree_node_moments.restype = None
         lib.ffo_tree_node_moments.argtypes = [vp] * 5
         lib.ffo_bh_eval.restype = i32
-        lib.ffo_bh_eval.argtypes = [vp, f32, i32, i64, vp, vp, vp, vp, i32]
+        lib.ffo_bh_eval.argtypes = [vp, f32, i32, i64, vp, vp, vp, vp, vp, i32]
         lib.ffo_bh_group_lists.restype = i32
         lib.ffo_bh_group_lists.argtypes = [vp, f32, i32, i64, vp, i64, vp, vp, i64, vp]
         _lib = lib
@@ -86,8 +86,9 @@ def pair(rk, uk, rj, uj):
     return h, f
 
 
-def allpairs(pos, mom, targets=None, nthreads: int = 0):
-    """All-pairs H, F (fp64).  targets: optional int64 index array -> rows follow it."""
+def allpairs(pos, mom, targets=None, nthreads: int = 0, scale: bool = False):
+    """All-pairs H, F (fp64).  targets: optional int64 index array -> rows follow it.
+    scale=True also returns Q (nt, 2): sqrt(sum_j |h_kj|^2), sqrt(sum_j |f_kj|^2), the error-metric scale."""
     pos, mom = _f32(pos), _f32(mom)
     N = pos.shape[0]
     if targets is None:
@@ -97,10 +98,12 @@ def allpairs(pos, mom, targets=None, nthreads: int = 0):
         nt, tp = targets.shape[0], targets.ctypes.data
     H = np.zeros((nt, 3))
     F = np.zeros((nt, 3))
-    rc = _load().ffo_allpairs(N, pos.ctypes.data, mom.ctypes.data, nt, tp, H.ctypes.data, F.ctypes.data, nthreads)
+    Q = np.zeros((nt, 2)) if scale else None
+    rc = _load().ffo_allpairs(N, pos.ctypes.data, mom.ctypes.data, nt, tp, H.ctypes.data, F.ctypes.data,
+                              Q.ctypes.data if scale else None, nthreads)
     if rc != 0:
         raise RuntimeError("ffo_allpairs failed")
-    return H, F
+    return (H, F, Q) if scale else (H, F)
 
 
 class Tree:
@@ -152,9 +155,10 @@ class Tree:
         self._lib.ffo_tree_node_moments(self._t, *[out[k].ctypes.data for k in ("sum_u", "sum_p", "mu", "cen")])
         return out
 
-    def eval(self, theta: float, W: int = 32, groups=None, nthreads: int = 0):
+    def eval(self, theta: float, W: int = 32, groups=None, nthreads: int = 0, scale: bool = False):
         """Barnes-Hut H, F (fp64, caller order, (N,3)); rows outside `groups` are NaN.
-        Returns (H, F, counters) with counters = (cell terms, particle terms, opening tests)."""
+        Returns (H, F, counters) with counters = (cell terms, particle terms, opening tests);
+        scale=True appends Q (N, 2), the per-target root-sum-square of the term magnitudes."""
         assert self._mom is not None, "call moments(mom) first"
         H = np.full((self.N, 3), np.nan)
         F = np.full((self.N, 3), np.nan)
@@ -164,11 +168,13 @@ class Tree:
         else:
             groups = np.ascontiguousarray(groups, dtype=np.int64)
             ng, gp = groups.shape[0], groups.ctypes.data
+        Q = np.full((self.N, 2), np.nan) if scale else None
         rc = self._lib.ffo_bh_eval(self._t, float(theta), int(W), ng, gp, H.ctypes.data, F.ctypes.data,
-                                   cnt.ctypes.data, nthreads)
+                                   Q.ctypes.data if scale else None, cnt.ctypes.data, nthreads)
         if rc != 0:
             raise RuntimeError("ffo_bh_eval failed")
-        return H, F, tuple(int(c) for c in cnt)
+        cnt = tuple(int(c) for c in cnt)
+        return (H, F, cnt, Q) if scale else (H, F, cnt)
 
     def group_lists(self, theta: float, W: int, g: int):
         """(accepted node indices, sorted slots reached through leaves) of group g."""
@@ -184,9 +190,10 @@ class Tree:
         return cells[: nc[0]].copy(), parts[: npart[0]].copy()
 
 
-def barnes_hut(pos, mom, theta: float, W: int = 32, nleaf: int = 1, groups=None, nthreads: int = 0):
-    """Convenience: build, moments, evaluate.  Returns (H, F, counters, tree)."""
+def barnes_hut(pos, mom, theta: float, W: int = 32, nleaf: int = 1, groups=None, nthreads: int = 0,
+               scale: bool = False):
+    """Convenience: build, moments, evaluate.  Returns (H, F, counters, tree) [+ (Q,) if scale]."""
     t = Tree(pos, nleaf)
     t.moments(mom)
-    H, F, cnt = t.eval(theta, W, groups, nthreads)
-    return H, F, cnt, t
+    out = t.eval(theta, W, groups, nthreads, scale)
+    return (out[0], out[1], out[2], t) + ((out[3],) if scale else ())

@@ -49,7 +49,7 @@
  */
 static void pair_accumulate(const double rk[3], const double uk[3],
                             const double rj[3], const double uj[3],
-                            double h[3], double f[3])
+                            double h[3], double f[3], double* q /* NULL or [2] */)
 {
     double rho[3] = { rk[0] - rj[0], rk[1] - rj[1], rk[2] - rj[2] };
     double r2 = rho[0] * rho[0] + rho[1] * rho[1] + rho[2] * rho[2];
@@ -59,11 +59,19 @@ static void pair_accumulate(const double rk[3], const double uk[3],
     double uj_rho = uj[0] * rho[0] + uj[1] * rho[1] + uj[2] * rho[2];
     double uk_rho = uk[0] * rho[0] + uk[1] * rho[1] + uk[2] * rho[2];
     double uj_uk = uj[0] * uk[0] + uj[1] * uk[1] + uj[2] * uk[2];
+    double th2 = 0.0, tf2 = 0.0;
     for (int a = 0; a < 3; ++a) {
-        h[a] += (3.0 * rho[a] * uj_rho - uj[a] * r2) / r5;
-        f[a] += 3.0 * (rho[a] * uj_uk + uk[a] * uj_rho + uj[a] * uk_rho) / r5
-                - 15.0 * rho[a] * uk_rho * uj_rho / r7;
+        double th = (3.0 * rho[a] * uj_rho - uj[a] * r2) / r5;
+        double tf = 3.0 * (rho[a] * uj_uk + uk[a] * uj_rho + uj[a] * uk_rho) / r5
+                    - 15.0 * rho[a] * uk_rho * uj_rho / r7;
+        h[a] += th;
+        f[a] += tf;
+        th2 += th * th; tf2 += tf * tf;
     }
+    /* not part of the method: the squared magnitudes of the terms, summed per target, give the
+     * scale Q_k = sqrt(sum_j |t_kj|^2) against which the tests measure rounding error when the
+     * terms of a sum cancel (error metric) */
+    if (q) { q[0] += th2; q[1] += tf2; }
 }
 
 /* public single-pair entry: h, f are OVERWRITTEN with the pair terms */
@@ -72,7 +80,7 @@ void ffo_pair(const double rk[3], const double uk[3], const double rj[3], const 
 {
     h[0] = h[1] = h[2] = 0.0;
     f[0] = f[1] = f[2] = 0.0;
-    pair_accumulate(rk, uk, rj, uj, h, f);
+    pair_accumulate(rk, uk, rj, uj, h, f, NULL);
 }
 
 static void widen3(const float* src, int64_t i, double out[3])
@@ -99,7 +107,8 @@ int ffo_max_threads(void) { return pick_threads(0); }
  * N) selects which k are evaluated; row t of H/F belongs to targets[t].
  */
 int ffo_allpairs(int64_t N, const float* pos, const float* mom,
-                 int64_t nt, const int64_t* targets, double* H, double* F, int nthreads)
+                 int64_t nt, const int64_t* targets, double* H, double* F, double* Q /* NULL or [nt][2] */,
+                 int nthreads)
 {
     if (N <= 0 || !pos || !mom || !H || !F) return -1;
     if (!targets) nt = N;
@@ -108,15 +117,16 @@ int ffo_allpairs(int64_t N, const float* pos, const float* mom,
 #pragma omp parallel for schedule(dynamic, 16) num_threads(nth)
     for (int64_t t = 0; t < nt; ++t) {
         int64_t k = targets ? targets[t] : t;
-        double rk[3], uk[3], h[3] = { 0, 0, 0 }, f[3] = { 0, 0, 0 };
+        double rk[3], uk[3], h[3] = { 0, 0, 0 }, f[3] = { 0, 0, 0 }, q[2] = { 0, 0 };
         widen3(pos, k, rk); widen3(mom, k, uk);
         for (int64_t j = 0; j < N; ++j) {
             if (j == k) continue;
             double rj[3], uj[3];
             widen3(pos, j, rj); widen3(mom, j, uj);
-            pair_accumulate(rk, uk, rj, uj, h, f);
+            pair_accumulate(rk, uk, rj, uj, h, f, q);
         }
         for (int a = 0; a < 3; ++a) { H[3 * t + a] = h[a]; F[3 * t + a] = f[a]; }
+        if (Q) { Q[2 * t] = sqrt(q[0]); Q[2 * t + 1] = sqrt(q[1]); }
     }
     return 0;
 }
@@ -387,6 +397,7 @@ typedef struct {
     float th2;
     int64_t g0, g1;           /* group = sorted slots [g0, g1) */
     double* h; double* f;     /* [g1-g0][3] accumulators (NULL when only listing) */
+    double* q;                /* [g1-g0][2] squared term magnitudes (error-metric scale) */
     uint64_t n_cell, n_part, n_mac;
     /* optional interaction lists (for tests) */
     int64_t* cells; int64_t n_cells_out, cap_cells;
@@ -419,7 +430,7 @@ static void visit(walk_ctx* w, int64_t id)
                 if (j == k) continue;                      /* Alg. 1 line 5 */
                 double rk[3], uk[3];
                 widen3(t->spos, k, rk); widen3(t->smom, k, uk);
-                pair_accumulate(rk, uk, rj, uj, w->h + 3 * (k - w->g0), w->f + 3 * (k - w->g0));
+                pair_accumulate(rk, uk, rj, uj, w->h + 3 * (k - w->g0), w->f + 3 * (k - w->g0), w->q + 2 * (k - w->g0));
                 w->n_part++;
             }
         }
@@ -442,7 +453,7 @@ static void visit(walk_ctx* w, int64_t id)
                 for (int64_t k = w->g0; k < w->g1; ++k) {
                     double rk[3], uk[3];
                     widen3(t->spos, k, rk); widen3(t->smom, k, uk);
-                    pair_accumulate(rk, uk, rj, uj, w->h + 3 * (k - w->g0), w->f + 3 * (k - w->g0));
+                    pair_accumulate(rk, uk, rj, uj, w->h + 3 * (k - w->g0), w->f + 3 * (k - w->g0), w->q + 2 * (k - w->g0));
                 }
                 w->n_cell += (uint64_t)(w->g1 - w->g0);
             }
@@ -462,7 +473,7 @@ static void visit(walk_ctx* w, int64_t id)
  * (group, internal node not holding a member) evaluated.
  */
 int ffo_bh_eval(const ffo_tree* t, float theta, int W, int64_t ng, const int64_t* groups,
-                double* H, double* F, uint64_t counters[3], int nthreads)
+                double* H, double* F, double* Q /* NULL or [N][2], caller order */, uint64_t counters[3], int nthreads)
 {
     if (!t || !t->has_moments || W < 1 || !(theta >= 0.0f) || !H || !F) return -1;
     int64_t n_groups = (t->N + W - 1) / W;
@@ -480,14 +491,19 @@ int ffo_bh_eval(const ffo_tree* t, float theta, int W, int64_t ng, const int64_t
         w.t = t; w.th2 = th2;
         w.g0 = g * W; w.g1 = w.g0 + W < t->N ? w.g0 + W : t->N;
         int64_t m = w.g1 - w.g0;
-        double* acc = (double*)calloc((size_t)m * 6, sizeof(double));
-        w.h = acc; w.f = acc + 3 * m;
+        double* acc = (double*)calloc((size_t)m * 8, sizeof(double));
+        w.h = acc; w.f = acc + 3 * m; w.q = acc + 6 * m;
         visit(&w, 0);
-        for (int64_t k = w.g0; k < w.g1; ++k)
+        for (int64_t k = w.g0; k < w.g1; ++k) {
             for (int a = 0; a < 3; ++a) {
                 H[3 * t->perm[k] + a] = w.h[3 * (k - w.g0) + a];
                 F[3 * t->perm[k] + a] = w.f[3 * (k - w.g0) + a];
             }
+            if (Q) {
+                Q[2 * t->perm[k]] = sqrt(w.q[2 * (k - w.g0)]);
+                Q[2 * t->perm[k] + 1] = sqrt(w.q[2 * (k - w.g0) + 1]);
+            }
+        }
         free(acc);
         c0 += w.n_cell; c1 += w.n_part; c2 += w.n_mac;
     }

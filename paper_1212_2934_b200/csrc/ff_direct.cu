@@ -61,26 +61,31 @@ ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n,
         __syncthreads();
         spos[t] = sp; smom[t] = sv;
         __syncthreads();
-        float hx = 0.f, hy = 0.f, hz = 0.f, fx = 0.f, fy = 0.f, fz = 0.f, sk = 0.f;
-        if (tile == blockIdx.x) {            // the only tile that holds this block's own targets
+        // fp32 partial sums over chunks of 32 sources, folded into the fp64 running sums: keeps the
+        // accumulation error at sqrt(32) ulp of a chunk sum instead of sqrt(N) ulp of the total
+        const bool own = tile == blockIdx.x;     // the only tile that holds this block's own targets
+        for (int c0 = 0; c0 < FF_DIRECT_THREADS; c0 += 32) {
+            float hx = 0.f, hy = 0.f, hz = 0.f, fx = 0.f, fy = 0.f, fz = 0.f, sk = 0.f;
+            if (own) {
 #pragma unroll 4
-            for (int i = 0; i < FF_DIRECT_THREADS; ++i) {
-                float4 a = spos[i], m = smom[i];
-                float dx = px - a.x, dy = py - a.y, dz = pz - a.z;
-                float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                float rinv = (i == t) ? 0.0f : ff_rsqrt_nr(r2);   // j + i != k (Alg. 1 line 5)
-                ff_pair_accum_d(dx, dy, dz, rinv, ux, uy, uz, m.x, m.y, m.z, hx, hy, hz, fx, fy, fz, sk);
-            }
-        } else {
+                for (int i = c0; i < c0 + 32; ++i) {
+                    float4 a = spos[i], m = smom[i];
+                    float dx = px - a.x, dy = py - a.y, dz = pz - a.z;
+                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    float rinv = (i == t) ? 0.0f : ff_rsqrt_nr(r2);   // j + i != k (Alg. 1 line 5)
+                    ff_pair_accum_d(dx, dy, dz, rinv, ux, uy, uz, m.x, m.y, m.z, hx, hy, hz, fx, fy, fz, sk);
+                }
+            } else {
 #pragma unroll 8
-            for (int i = 0; i < FF_DIRECT_THREADS; ++i) {
-                float4 a = spos[i], m = smom[i];
-                float dx = px - a.x, dy = py - a.y, dz = pz - a.z;
-                float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                ff_pair_accum_d(dx, dy, dz, ff_rsqrt_nr(r2), ux, uy, uz, m.x, m.y, m.z, hx, hy, hz, fx, fy, fz, sk);
+                for (int i = c0; i < c0 + 32; ++i) {
+                    float4 a = spos[i], m = smom[i];
+                    float dx = px - a.x, dy = py - a.y, dz = pz - a.z;
+                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    ff_pair_accum_d(dx, dy, dz, ff_rsqrt_nr(r2), ux, uy, uz, m.x, m.y, m.z, hx, hy, hz, fx, fy, fz, sk);
+                }
             }
+            acc[0] += hx; acc[1] += hy; acc[2] += hz; acc[3] += fx; acc[4] += fy; acc[5] += fz; acc[6] += sk;
         }
-        acc[0] += hx; acc[1] += hy; acc[2] += hz; acc[3] += fx; acc[4] += fy; acc[5] += fz; acc[6] += sk;
     }
     if (k >= n) return;
     acc[3] += acc[6] * (double)ux; acc[4] += acc[6] * (double)uy; acc[5] += acc[6] * (double)uz;

@@ -124,13 +124,32 @@ def canonical_from_oracle(tree):
             zip(nd["first"], nd["level"], nd["prefix"], nd["count"], nd["is_leaf"])]
 
 
-# ---- error metric of DESIGN.md ---------------------------------
-def rel_err(x, ref):
-    """Per-particle relative L2 error with the 1e-3*rms floor; returns (max, median, p99, global)."""
+# ---- error metric of DESIGN.md ("error metric", reading Q19) ------------------
+KAPPA = 8.0
+
+
+def rel_err(x, ref, Q=None):
+    """Per-particle relative L2 error e_k = |x_k - ref_k| / max(|ref_k|, floor_k).
+
+    floor_k = Q_k / KAPPA with Q_k = sqrt(sum_j |t_kj|^2), the root-sum-square of the terms of
+    particle k's own sum (from the oracle): a sum whose terms cancel below 1/KAPPA of their
+    natural scale is measured against that scale, because fp32 rounding error is proportional to
+    the size of the TERMS, not of their sum.  Without Q: floor = 1e-3 * rms_k |ref|.
+    Returns (max, median, p99, global relative L2)."""
     x = np.asarray(x, np.float64)
     ref = np.asarray(ref, np.float64)
     nr = np.linalg.norm(ref, axis=1)
-    rms = np.sqrt((nr**2).mean())
-    e = np.linalg.norm(x - ref, axis=1) / np.maximum(nr, 1e-3 * rms)
-    glob = np.linalg.norm(x - ref) / np.linalg.norm(ref)
+    if Q is None:
+        floor = 1e-3 * np.sqrt((nr**2).mean())
+    else:
+        floor = np.asarray(Q, np.float64) / KAPPA
+    e = np.linalg.norm(x - ref, axis=1) / np.maximum(np.maximum(nr, floor), 1e-300)
+    glob = np.linalg.norm(x - ref) / max(np.linalg.norm(ref), 1e-300)
     return float(e.max()), float(np.median(e)), float(np.percentile(e, 99)), float(glob)
+
+
+def check_hf(H, F, Ho, Fo, Q, tol):
+    """Assert both fields within tol under the metric above; returns the two error tuples."""
+    eh, ef = rel_err(H, Ho, Q[:, 0]), rel_err(F, Fo, Q[:, 1])
+    assert eh[0] <= tol and ef[0] <= tol, (eh, ef)
+    return eh, ef

@@ -1,9 +1,9 @@
 """Parity of the CUDA path (through the C ABI) against the oracle, element by element.
 
-Tolerances (BASELINE.json north_star, metric of DESIGN.md / SURVEY Q19):
+Tolerances (BASELINE.json north_star; error metric of DESIGN.md, reading Q19):
   Barnes-Hut vs oracle Barnes-Hut (same theta, same tree, same group rule) ... max_k e_k <= 1e-4
   direct vs oracle all-pairs ................................................. max_k e_k <= 1e-5
-  e_k = |x_k - ref_k|_2 / max(|ref_k|_2, 1e-3 rms_k |ref|_2)
+  e_k = |x_k - ref_k|_2 / max(|ref_k|_2, Q_k / 8),  Q_k = sqrt(sum_j |term_kj|^2) from the oracle
   keys, permutation, root cube, cell topology, cell centres/moments .......... bit exact
 """
 import numpy as np
@@ -11,7 +11,7 @@ import pytest
 
 import ffgen
 import oracle
-from helpers import canonical_from_oracle, rel_err
+from helpers import canonical_from_oracle, check_hf, rel_err
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -67,19 +67,17 @@ def test_config1_direct_vs_allpairs(ff, cfg1):
     pos, mom = cfg1["pos"], cfg1["mom"]
     ctx = ff.FFContext(len(pos), 0.5)
     H, F = ctx.eval_direct(_dev(pos), _dev(mom))
-    Ho, Fo = oracle.allpairs(pos, mom)
-    eh, ef = rel_err(H.cpu().numpy(), Ho), rel_err(F.cpu().numpy(), Fo)
-    assert eh[0] <= TOL_DIRECT and ef[0] <= TOL_DIRECT, (eh, ef)
+    Ho, Fo, Q = oracle.allpairs(pos, mom, scale=True)
+    check_hf(H.cpu().numpy(), F.cpu().numpy(), Ho, Fo, Q, TOL_DIRECT)
 
 
 def test_config1_tree_bit_exact_and_bh_parity(ff, cfg1):
     pos, mom = cfg1["pos"], cfg1["mom"]
     ctx, H, F = _gpu_bh(ff, pos, mom, cfg1["theta"])
-    Ho, Fo, cnt, otree = oracle.barnes_hut(pos, mom, cfg1["theta"], 32)
+    Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, cfg1["theta"], 32, scale=True)
     _check_tree(ff, ctx, otree, otree.moments(mom))
     assert ctx.counters() == cnt                      # identical interaction sets
-    eh, ef = rel_err(H, Ho), rel_err(F, Fo)
-    assert eh[0] <= TOL_BH and ef[0] <= TOL_BH, (eh, ef)
+    check_hf(H, F, Ho, Fo, Q, TOL_BH)
 
 
 def test_config1_host_entry_points(ff, cfg1):
@@ -87,11 +85,11 @@ def test_config1_host_entry_points(ff, cfg1):
     ctx = ff.FFContext(len(pos), 0.5)
     H, F = np.empty_like(pos), np.empty_like(pos)
     ctx.eval_bh_host(pos, mom, H, F)
-    Ho, Fo, _, _ = oracle.barnes_hut(pos, mom, 0.5, 32)
-    assert rel_err(H, Ho)[0] <= TOL_BH and rel_err(F, Fo)[0] <= TOL_BH
+    Ho, Fo, _, _, Q = oracle.barnes_hut(pos, mom, 0.5, 32, scale=True)
+    check_hf(H, F, Ho, Fo, Q, TOL_BH)
     ctx.eval_direct_host(pos, mom, H, F)
-    Ha, Fa = oracle.allpairs(pos, mom)
-    assert rel_err(H, Ha)[0] <= TOL_DIRECT and rel_err(F, Fa)[0] <= TOL_DIRECT
+    Ha, Fa, Qa = oracle.allpairs(pos, mom, scale=True)
+    check_hf(H, F, Ha, Fa, Qa, TOL_DIRECT)
 
 
 # ------------------------------------------------- ragged sizes, edge cases ----
@@ -100,17 +98,19 @@ def test_ragged_sizes(ff, N):
     c = ffgen.config(1, N=N, seed=N)
     pos, mom = c["pos"], c["mom"]
     ctx, H, F = _gpu_bh(ff, pos, mom, 0.5)
-    Ho, Fo, cnt, otree = oracle.barnes_hut(pos, mom, 0.5, 32)
+    Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, 0.5, 32, scale=True)
     _check_tree(ff, ctx, otree, otree.moments(mom))
     assert ctx.counters() == cnt
     if N > 1:
-        assert rel_err(H, Ho)[0] <= TOL_BH and rel_err(F, Fo)[0] <= TOL_BH
+        check_hf(H, F, Ho, Fo, Q, TOL_BH)
     else:
         assert np.all(H == 0) and np.all(F == 0)
     Hd, Fd = ctx.eval_direct(_dev(pos), _dev(mom))
-    Ha, Fa = oracle.allpairs(pos, mom)
+    Ha, Fa, Qa = oracle.allpairs(pos, mom, scale=True)
     if N > 1:
-        assert rel_err(Hd.cpu().numpy(), Ha)[0] <= TOL_DIRECT and rel_err(Fd.cpu().numpy(), Fa)[0] <= TOL_DIRECT
+        check_hf(Hd.cpu().numpy(), Fd.cpu().numpy(), Ha, Fa, Qa, TOL_DIRECT)
+    else:
+        assert np.all(Hd.cpu().numpy() == 0) and np.all(Fd.cpu().numpy() == 0)
 
 
 @pytest.mark.parametrize("nleaf", [1, 2, 8, 32, 100])
@@ -118,10 +118,10 @@ def test_leaf_capacity(ff, nleaf):
     c = ffgen.config(1, N=1500, seed=3)
     pos, mom = c["pos"], c["mom"]
     ctx, H, F = _gpu_bh(ff, pos, mom, 0.6, nleaf=nleaf)
-    Ho, Fo, cnt, otree = oracle.barnes_hut(pos, mom, 0.6, 32, nleaf=nleaf)
+    Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, 0.6, 32, nleaf=nleaf, scale=True)
     _check_tree(ff, ctx, otree, otree.moments(mom))
     assert ctx.counters() == cnt
-    assert rel_err(H, Ho)[0] <= TOL_BH and rel_err(F, Fo)[0] <= TOL_BH
+    check_hf(H, F, Ho, Fo, Q, TOL_BH)
 
 
 def test_theta_zero_equals_all_pairs(ff):
@@ -129,8 +129,8 @@ def test_theta_zero_equals_all_pairs(ff):
     pos, mom = c["pos"], c["mom"]
     ctx, H, F = _gpu_bh(ff, pos, mom, 0.0)
     assert ctx.counters()[:2] == (0, 1200 * 1199)
-    Ha, Fa = oracle.allpairs(pos, mom)
-    assert rel_err(H, Ha)[0] <= TOL_BH and rel_err(F, Fa)[0] <= TOL_BH
+    Ha, Fa, Qa = oracle.allpairs(pos, mom, scale=True)
+    check_hf(H, F, Ha, Fa, Qa, TOL_BH)
 
 
 def test_root_is_leaf_when_n_le_nleaf(ff):
@@ -138,8 +138,8 @@ def test_root_is_leaf_when_n_le_nleaf(ff):
     pos, mom = c["pos"], c["mom"]
     ctx, H, F = _gpu_bh(ff, pos, mom, 0.5, nleaf=64)
     assert ctx.get_tree()["n_cells"] == 0 and ctx.counters() == (0, 40 * 39, 0)
-    Ha, Fa = oracle.allpairs(pos, mom)
-    assert rel_err(H, Ha)[0] <= TOL_BH and rel_err(F, Fa)[0] <= TOL_BH
+    Ha, Fa, Qa = oracle.allpairs(pos, mom, scale=True)
+    check_hf(H, F, Ha, Fa, Qa, TOL_BH)
 
 
 def test_depth_cap_and_same_octant_chain(ff):
@@ -151,11 +151,11 @@ def test_depth_cap_and_same_octant_chain(ff):
     pos = np.vstack([blob, [[100.0, 100.0, 100.0]], [[60.0, 10.0, 30.0]]]).astype(np.float32)
     mom = ffgen.moments_isotropic(len(pos), 2)
     ctx, H, F = _gpu_bh(ff, pos, mom, 0.5)
-    Ho, Fo, cnt, otree = oracle.barnes_hut(pos, mom, 0.5, 32)
+    Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, 0.5, 32, scale=True)
     assert otree.nodes()["level"].max() == 10 and (otree.nodes()["count"][otree.nodes()["is_leaf"] == 1] > 1).any()
     _check_tree(ff, ctx, otree, otree.moments(mom))
     assert ctx.counters() == cnt
-    assert rel_err(H, Ho)[0] <= TOL_BH and rel_err(F, Fo)[0] <= TOL_BH
+    check_hf(H, F, Ho, Fo, Q, TOL_BH)
 
 
 def test_eight_corners_and_coplanar(ff):
@@ -165,10 +165,10 @@ def test_eight_corners_and_coplanar(ff):
     for pos in (corners, plane):
         mom = ffgen.moments_isotropic(len(pos), 1)
         ctx, H, F = _gpu_bh(ff, pos, mom, 0.5)
-        Ho, Fo, cnt, otree = oracle.barnes_hut(pos, mom, 0.5, 32)
+        Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, 0.5, 32, scale=True)
         _check_tree(ff, ctx, otree, otree.moments(mom))
         assert ctx.counters() == cnt
-        assert rel_err(H, Ho)[0] <= TOL_BH and rel_err(F, Fo)[0] <= TOL_BH
+        check_hf(H, F, Ho, Fo, Q, TOL_BH)
 
 
 def test_context_reuse_and_smaller_n(ff):
@@ -178,9 +178,9 @@ def test_context_reuse_and_smaller_n(ff):
         p, m = _dev(c["pos"]), _dev(c["mom"])
         ctx.build_tree(p)
         H, F = ctx.eval_bh(p, m)
-        Ho, Fo, cnt, _ = oracle.barnes_hut(c["pos"], c["mom"], 0.5, 32)
+        Ho, Fo, cnt, _, Q = oracle.barnes_hut(c["pos"], c["mom"], 0.5, 32, scale=True)
         assert ctx.counters() == cnt
-        assert rel_err(H.cpu().numpy(), Ho)[0] <= TOL_BH and rel_err(F.cpu().numpy(), Fo)[0] <= TOL_BH
+        check_hf(H.cpu().numpy(), F.cpu().numpy(), Ho, Fo, Q, TOL_BH)
 
 
 def test_error_codes(ff):
@@ -211,15 +211,15 @@ def test_config2_theta_sweep(ff):
     Hd, Fd = Hd.cpu().numpy(), Fd.cpu().numpy()
     # direct vs oracle all-pairs on sampled targets (full all-pairs on 65 536 would take minutes on the host)
     tg = np.random.default_rng(0).choice(len(pos), 2048, replace=False)
-    Ha, Fa = oracle.allpairs(pos, mom, targets=tg)
-    assert rel_err(Hd[tg], Ha)[0] <= TOL_DIRECT and rel_err(Fd[tg], Fa)[0] <= TOL_DIRECT
+    Ha, Fa, Qa = oracle.allpairs(pos, mom, targets=tg, scale=True)
+    check_hf(Hd[tg], Fd[tg], Ha, Fa, Qa, TOL_DIRECT)
     prev = None
     for theta in c["thetas"]:
         ctx.set_option(ff.FF_OPT_THETA, theta)
         H, F = ctx.eval_bh(p, m)
-        Ho, Fo, cnt, = otree.eval(theta, 32)
+        Ho, Fo, cnt, Q = otree.eval(theta, 32, scale=True)
         assert ctx.counters() == cnt
-        assert rel_err(H.cpu().numpy(), Ho)[0] <= TOL_BH and rel_err(F.cpu().numpy(), Fo)[0] <= TOL_BH
+        check_hf(H.cpu().numpy(), F.cpu().numpy(), Ho, Fo, Q, TOL_BH)
         # approximation error vs all-pairs grows with theta (reported by bench.py; parity unpinned by the paper)
         err = rel_err(H.cpu().numpy(), Hd)[3]
         assert prev is None or err > prev
@@ -248,13 +248,10 @@ def _sampled_parity(ff, c, n_groups, seed=0):
     assert np.array_equal(t["cell_end"], (nd["first"] + nd["count"])[internal].astype(np.int32))
     assert np.array_equal(t["cell_level"], nd["level"][internal])
     groups = np.random.default_rng(seed).choice((N + 31) // 32, n_groups, replace=False)
-    Ho, Fo, _ = otree.eval(theta, 32, groups=groups)
+    Ho, Fo, _, Q = otree.eval(theta, 32, groups=groups, scale=True)
     rows = operm[(groups[:, None] * 32 + np.arange(32)[None, :]).ravel()]
-    scale_h = np.sqrt((np.linalg.norm(Ho[rows], axis=1) ** 2).mean())
-    eh = np.linalg.norm(H[rows] - Ho[rows], axis=1) / np.maximum(np.linalg.norm(Ho[rows], axis=1), 1e-3 * scale_h)
-    scale_f = np.sqrt((np.linalg.norm(Fo[rows], axis=1) ** 2).mean())
-    ef = np.linalg.norm(F[rows] - Fo[rows], axis=1) / np.maximum(np.linalg.norm(Fo[rows], axis=1), 1e-3 * scale_f)
-    assert eh.max() <= TOL_BH and ef.max() <= TOL_BH, (eh.max(), ef.max())
+    rows = rows[rows < N]
+    check_hf(H[rows], F[rows], Ho[rows], Fo[rows], Q[rows], TOL_BH)
     assert np.isfinite(H).all() and np.isfinite(F).all()
     return ctx, H, F
 
@@ -267,3 +264,8 @@ def test_config3_one_million_sampled(ff):
 
 def test_config4_chains_sampled(ff):
     _sampled_parity(ff, ffgen.config(4), 256)
+
+
+def test_config5_sixteen_million_sampled(ff):
+    # N = 2^24, phi = 0.2, theta = 0.6: the HBM-resident case; the oracle walks 64 sampled groups
+    _sampled_parity(ff, ffgen.config(5), 64)
