@@ -171,7 +171,7 @@ ff_k_cells_fill(const uint32_t* __restrict__ key, int n, int nleaf, const int32_
 // ((c0 + c1) + c2) + ...; a leaf's particles left to right; one fp64 divide and a
 // single rounding to fp32.
 __global__ void __launch_bounds__(128)
-ff_k_moments_level(int level, const ff_globals* __restrict__ g, const int32_t* __restrict__ cell_first,
+ff_k_moments_level(int level, ff_globals* __restrict__ g, const int32_t* __restrict__ cell_first,
                    const int32_t* __restrict__ cell_end, const int32_t* __restrict__ cell_level,
                    const int32_t* __restrict__ cell_child, const int32_t* __restrict__ leaf_count,
                    const float4* __restrict__ pos_s, const float4* __restrict__ mom_s,
@@ -179,6 +179,7 @@ ff_k_moments_level(int level, const ff_globals* __restrict__ g, const int32_t* _
                    float4* __restrict__ centre, float4* __restrict__ moment)
 {
     int n_cells = g->n_cells;
+    if (level == 0 && blockIdx.x == 0 && threadIdx.x == 0) g->walk_next = 0;   // last launch before the walk
     float s = ldexpf(g->S, -level);
     float s2 = __fmul_rn(s, s);
     for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < n_cells; id += gridDim.x * blockDim.x) {

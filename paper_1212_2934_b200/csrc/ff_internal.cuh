@@ -24,7 +24,7 @@
 #define FF_SCAN_TILE (FF_SCAN_THREADS * FF_SCAN_ITEMS)
 
 // ---- walk geometry (ff_walk.cu) ---------------------------------------------
-#define FF_WALK_WARPS 8            // warps (= target groups) per block
+#define FF_WALK_WARPS 4            // warps (= target groups) per block
 #define FF_WALK_STACK 1024         // traversal stack entries per warp
 #define FF_WALK_PEND 64            // pending interaction ring per warp (two batches of 32)
 
@@ -41,7 +41,7 @@ struct ff_globals {
     float inv;                // fl(1024 / S)
     int32_t n_cells;          // internal cells of the current tree
     int32_t error;            // sticky device-side error flag (FF_ERR_*)
-    int32_t pad0;
+    int32_t walk_next;        // next target group of the persistent walk (zeroed by the level-0 moment launch)
     unsigned long long counters[3];   // n_cell, n_particle, n_mac (FF_OPT_COUNTERS)
     uint32_t digit_total[FF_RADIX];   // per-pass digit totals (ff_sort.cu)
 };

@@ -14,47 +14,101 @@
 //                     for its OWN target: a dense, branch-free loop of Eq. 11 / Eq. 12
 //                      fed by broadcast float4 shared-memory reads.
 //
-// Both produce exactly the interaction set of the oracle's recursive walk; only
-// the summation order differs.  fp32 arithmetic; the opening test uses explicit
-// round-to-nearest intrinsics so it is bit-identical to the oracle's.
+// Blackwell specific: the evaluation and the opening test are written with the
+// packed FP32 instructions of sm_100 (FFMA2 / FMUL2 / FADD2 through __ffma2_rn,
+// __fmul2_rn, __fadd2_rn): one lane handles TWO sources (or two group members)
+// per instruction.  The FP32 pipe does the same work, but it needs half the
+// issue slots, and issue was the limiter of the scalar version (profiles/).  The
+// ring therefore stores sources as PAIRS: (x0,x1,y0,y1) (z0,z1,mx0,mx1)
+// (my0,my1,mz0,mz1), three broadcast LDS.128 per two sources.
+//
+// Both phases produce exactly the interaction set of the oracle's recursive walk;
+// only the summation order differs.  fp32 arithmetic; the opening test uses
+// round-to-nearest intrinsics in the oracle's operation order, so every decision
+// is bit-identical to the oracle's.
 #include "ff_internal.cuh"
+
+#define FF_PEND_PAIRS (FF_WALK_PEND / 2)
 
 struct ff_walk_smem {
     int32_t stack[FF_WALK_STACK];
-    float4 pend_pos[FF_WALK_PEND];
-    float4 pend_mom[FF_WALK_PEND];
-    float4 mem_pos[32];
+    float4 pend[FF_PEND_PAIRS * 3];    // pair p: [3p] = x0,x1,y0,y1  [3p+1] = z0,z1,mx0,mx1  [3p+2] = my0,my1,mz0,mz1
+    float4 mem_xy[16];                 // group members, pair m: x0,x1,y0,y1
+    float2 mem_z[16];                  //                        z0,z1
 };
 
-// One source term of Eq. 11 (h) and Eq. 12 (f) for target (p, u).  The u_k term of
-// Eq. 12 is accumulated as a scalar (sk) and multiplied by u_k once at the end.
-// rinv must already be 1/|rho| (0 for a term that is to be skipped).
-__device__ __forceinline__ void ff_pair_accum(float dx, float dy, float dz, float rinv, float ux, float uy, float uz,
-                                              float mx, float my, float mz, float& hx, float& hy, float& hz, float& fx,
-                                              float& fy, float& fz, float& sk)
+__device__ __forceinline__ float2 ff_dup(float a) { return make_float2(a, a); }
+
+// MUFU.RSQ without the denormal pre/post-scaling of rsqrtf (2 FSETP + 4 FMUL per pair of sources):
+// r^2 of two distinct particles is never denormal for inputs the ABI allows.
+__device__ __forceinline__ float ff_rsqrt(float x)
 {
-    float rinv2 = rinv * rinv;
-    float rinv3 = rinv2 * rinv;
-    float r5x3 = 3.0f * (rinv3 * rinv2);                 // 3 / r^5
-    float a = fmaf(mz, dz, fmaf(my, dy, mx * dx));       // u_j . rho
-    float b = fmaf(uz, dz, fmaf(uy, dy, ux * dx));       // u_k . rho
-    float cc = fmaf(mz, uz, fmaf(my, uy, mx * ux));      // u_j . u_k
-    float ca = a * r5x3;                                 // 3 (u_j.rho) / r^5
-    float cb = b * r5x3;                                 // 3 (u_k.rho) / r^5
-    // h += 3 rho (u_j.rho)/r^5 - u_j / r^3
-    hx = fmaf(ca, dx, hx); hy = fmaf(ca, dy, hy); hz = fmaf(ca, dz, hz);
-    hx = fmaf(-rinv3, mx, hx); hy = fmaf(-rinv3, my, hy); hz = fmaf(-rinv3, mz, hz);
-    // f += rho [3 (u_j.u_k) - 15 (u_j.rho)(u_k.rho)/r^2]/r^5 + u_k ca + u_j cb
-    float t = (a * b) * rinv2;
-    float cr = fmaf(-5.0f, t, cc) * r5x3;
-    fx = fmaf(cr, dx, fx); fy = fmaf(cr, dy, fy); fz = fmaf(cr, dz, fz);
-    fx = fmaf(cb, mx, fx); fy = fmaf(cb, my, fy); fz = fmaf(cb, mz, fz);
-    sk += ca;
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 }
 
+// target-side registers of one lane: position and moment duplicated into both halves of a pair
+struct ff_target2 {
+    float2 px, py, pz, ux, uy, uz;
+};
+
+// running sums of one lane, even / odd sources in the two halves; f = fv + sk u_k (the u_k term
+// of Eq. 12 is accumulated as a scalar and applied once at the end).  The two parts of Eq. 11 go
+// into ONE accumulator: for aligned moments sum 3 rho (u.rho)/r^5 and sum u/r^3 are each far larger
+// than their difference, and separate fp32 sums would lose that difference to rounding.
+struct ff_acc2 {
+    float2 hx, hy, hz, fx, fy, fz, sk;
+};
+
+// Two source terms of Eq. 11 (h) and Eq. 12 (f) for one target.  q0,q1,q2 = the pair's three
+// float4 of the ring; rinv = 1/|rho| per half (0 for a term that is to be skipped).
+//   h_kj = 3 rho (u_j.rho)/r^5 - u_j/r^3
+//   f_kj = { rho [(u_j.u_k) - 5 (u_j.rho)(u_k.rho)/r^2] + u_k (u_j.rho) + u_j (u_k.rho) } 3/r^5
+__device__ __forceinline__ void ff_pair2_geom(const float4& q0, const float4& q1, const ff_target2& t, float2& dx,
+                                              float2& dy, float2& dz, float2& r2)
+{
+    const float2 neg1 = ff_dup(-1.0f);
+    dx = __ffma2_rn(make_float2(q0.x, q0.y), neg1, t.px);    // rho = p_k - p_j (one rounding, as a subtraction)
+    dy = __ffma2_rn(make_float2(q0.z, q0.w), neg1, t.py);
+    dz = __ffma2_rn(make_float2(q1.x, q1.y), neg1, t.pz);
+    r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+}
+
+__device__ __forceinline__ void ff_pair2_accum(const float4& q1, const float4& q2, const ff_target2& t, float2 dx,
+                                               float2 dy, float2 dz, float2 rinv, ff_acc2& s)
+{
+    const float2 mx = make_float2(q1.z, q1.w), my = make_float2(q2.x, q2.y), mz = make_float2(q2.z, q2.w);
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 rinv3 = __fmul2_rn(rinv2, rinv);
+    const float2 r5 = __fmul2_rn(rinv3, __fmul2_rn(rinv2, ff_dup(3.0f)));         // 3 / r^5
+    const float2 a = __ffma2_rn(mz, dz, __ffma2_rn(my, dy, __fmul2_rn(mx, dx)));   // u_j . rho
+    const float2 b = __ffma2_rn(t.uz, dz, __ffma2_rn(t.uy, dy, __fmul2_rn(t.ux, dx)));   // u_k . rho
+    const float2 c = __ffma2_rn(mz, t.uz, __ffma2_rn(my, t.uy, __fmul2_rn(mx, t.ux)));   // u_j . u_k
+    const float2 ca = __fmul2_rn(a, r5);
+    const float2 cb = __fmul2_rn(b, r5);
+    const float2 nr3 = __fmul2_rn(rinv2, make_float2(-rinv.x, -rinv.y));           // -1 / r^3 (negation folds into the operand)
+    s.hx = __ffma2_rn(ca, dx, s.hx); s.hy = __ffma2_rn(ca, dy, s.hy); s.hz = __ffma2_rn(ca, dz, s.hz);
+    s.hx = __ffma2_rn(nr3, mx, s.hx); s.hy = __ffma2_rn(nr3, my, s.hy); s.hz = __ffma2_rn(nr3, mz, s.hz);
+    const float2 w = __fmul2_rn(__fmul2_rn(ca, b), rinv2);                         // 3 (u_j.rho)(u_k.rho) / r^7
+    const float2 cr = __ffma2_rn(ff_dup(-5.0f), w, __fmul2_rn(c, r5));
+    s.fx = __ffma2_rn(cr, dx, s.fx); s.fy = __ffma2_rn(cr, dy, s.fy); s.fz = __ffma2_rn(cr, dz, s.fz);
+    s.fx = __ffma2_rn(cb, mx, s.fx); s.fy = __ffma2_rn(cb, my, s.fy); s.fz = __ffma2_rn(cb, mz, s.fz);
+    s.sk = __fadd2_rn(s.sk, ca);
+}
+
+// write one interaction (A = position, B = moment) to ring slot `slot`
+__device__ __forceinline__ void ff_ring_store(ff_walk_smem& sm, int slot, const float4& A, const float4& B)
+{
+    float* f = reinterpret_cast<float*>(sm.pend) + (slot >> 1) * 12 + (slot & 1);
+    f[0] = A.x; f[2] = A.y; f[4] = A.z; f[6] = B.x; f[8] = B.y; f[10] = B.z;
+}
+
+// one group of 32 consecutive sorted targets, walked by one warp
 template <bool COUNT>
-__global__ void __launch_bounds__(FF_WALK_WARPS * 32)
-ff_k_walk(int n, float theta, const ff_globals* __restrict__ g, const float4* __restrict__ pos_s,
+__device__ __forceinline__ void
+ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
+          int n, float theta, const int n_cells, const float4* __restrict__ pos_s,
           const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
           const int32_t* __restrict__ cell_first,
           const int32_t* __restrict__ cell_end, const int4* __restrict__ cell_child,
@@ -62,12 +116,7 @@ ff_k_walk(int n, float theta, const ff_globals* __restrict__ g, const float4* __
           const float4* __restrict__ moment, float* __restrict__ H_out, float* __restrict__ F_out,
           unsigned long long* __restrict__ counters)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    ff_walk_smem& sm = reinterpret_cast<ff_walk_smem*>(smem_raw)[w];
-    const int grp = blockIdx.x * FF_WALK_WARPS + w;
     const int g0 = grp * 32;
-    if (g0 >= n) return;                                   // whole warp
     const int g1 = min(n, g0 + 32);
     const int nm = g1 - g0;
     const unsigned lt = (1u << lane) - 1u;
@@ -75,46 +124,57 @@ ff_k_walk(int n, float theta, const ff_globals* __restrict__ g, const float4* __
     // own target (lanes past the end duplicate the last member; their results are dropped)
     const int k = g0 + min(lane, nm - 1);
     const float4 pk = __ldg(pos_s + k), uk = __ldg(mom_s + k);
-    const float px = pk.x, py = pk.y, pz = pk.z, ux = uk.x, uy = uk.y, uz = uk.z;
-    float hx = 0.f, hy = 0.f, hz = 0.f, fx = 0.f, fy = 0.f, fz = 0.f, sk = 0.f;
+    ff_target2 tg;
+    tg.px = ff_dup(pk.x); tg.py = ff_dup(pk.y); tg.pz = ff_dup(pk.z);
+    tg.ux = ff_dup(uk.x); tg.uy = ff_dup(uk.y); tg.uz = ff_dup(uk.z);
+    ff_acc2 s;
+    s.hx = s.hy = s.hz = s.fx = s.fy = s.fz = s.sk = ff_dup(0.0f);
     unsigned long long c_cell = 0, c_part = 0, c_mac = 0;
 
-    sm.mem_pos[lane] = pk;
-    sm.pend_pos[lane] = pk;
-    sm.pend_mom[lane] = uk;
+    {   // group members in pair layout for the opening test; the ring's first batch = the members themselves
+        float* mxy = reinterpret_cast<float*>(sm.mem_xy) + (lane >> 1) * 4 + (lane & 1);
+        mxy[0] = pk.x; mxy[2] = pk.y;
+        reinterpret_cast<float*>(sm.mem_z)[lane] = pk.z;
+        ff_ring_store(sm, lane, pk, uk);
+    }
     __syncwarp();
-    // the group's own members: direct terms, self skipped by index (Alg. 1 line 5)
-    for (int j = 0; j < nm; ++j) {
-        float4 sp = sm.pend_pos[j], sv = sm.pend_mom[j];
-        float dx = px - sp.x, dy = py - sp.y, dz = pz - sp.z;
-        float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-        float rinv = (j == lane) ? 0.0f : rsqrtf(r2);
-        ff_pair_accum(dx, dy, dz, rinv, ux, uy, uz, sv.x, sv.y, sv.z, hx, hy, hz, fx, fy, fz, sk);
+    // the group's own members: direct terms, self skipped by index (Alg. 1 line 5);
+    // slots >= nm of a ragged last group hold copies of the last member and are masked the same way
+#pragma unroll 2
+    for (int jj = 0; jj < 16; ++jj) {
+        const float4 q0 = sm.pend[3 * jj], q1 = sm.pend[3 * jj + 1], q2 = sm.pend[3 * jj + 2];
+        float2 dx, dy, dz, r2;
+        ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
+        float2 rinv;
+        rinv.x = (2 * jj == lane || 2 * jj >= nm) ? 0.0f : ff_rsqrt(r2.x);
+        rinv.y = (2 * jj + 1 == lane || 2 * jj + 1 >= nm) ? 0.0f : ff_rsqrt(r2.y);
+        ff_pair2_accum(q1, q2, tg, dx, dy, dz, rinv, s);
     }
     if (COUNT) c_part += (unsigned long long)nm * (unsigned long long)(nm - 1);
     __syncwarp();
 
     const float th2 = __fmul_rn(theta, theta);
-    int pend_head = 0, pend_cnt = 0;                       // warp-uniform ring state
+    int pend_head = 0, pend_cnt = 0;                       // warp-uniform ring state (entries)
     int sp_top = 0;                                        // warp-uniform stack size
 
-    // evaluate `cnt` pending entries starting at pend_head for this lane's target
-    auto eval = [&](int cnt) {
+    // evaluate `pairs` pending source pairs starting at ring entry pend_head for this lane's target
+    auto eval = [&](int pairs) {
         __syncwarp();
-        if (cnt == 32) {
-#pragma unroll 8
-            for (int j = 0; j < 32; ++j) {
-                float4 sp = sm.pend_pos[pend_head + j], sv = sm.pend_mom[pend_head + j];
-                float dx = px - sp.x, dy = py - sp.y, dz = pz - sp.z;
-                float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                ff_pair_accum(dx, dy, dz, rsqrtf(r2), ux, uy, uz, sv.x, sv.y, sv.z, hx, hy, hz, fx, fy, fz, sk);
+        const float4* q = sm.pend + 3 * (pend_head >> 1);
+        if (pairs == 16) {
+#pragma unroll 4
+            for (int jj = 0; jj < 16; ++jj) {
+                const float4 q0 = q[3 * jj], q1 = q[3 * jj + 1], q2 = q[3 * jj + 2];
+                float2 dx, dy, dz, r2;
+                ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
+                ff_pair2_accum(q1, q2, tg, dx, dy, dz, make_float2(ff_rsqrt(r2.x), ff_rsqrt(r2.y)), s);
             }
         } else {
-            for (int j = 0; j < cnt; ++j) {
-                float4 sp = sm.pend_pos[pend_head + j], sv = sm.pend_mom[pend_head + j];
-                float dx = px - sp.x, dy = py - sp.y, dz = pz - sp.z;
-                float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                ff_pair_accum(dx, dy, dz, rsqrtf(r2), ux, uy, uz, sv.x, sv.y, sv.z, hx, hy, hz, fx, fy, fz, sk);
+            for (int jj = 0; jj < pairs; ++jj) {
+                const float4 q0 = q[3 * jj], q1 = q[3 * jj + 1], q2 = q[3 * jj + 2];
+                float2 dx, dy, dz, r2;
+                ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
+                ff_pair2_accum(q1, q2, tg, dx, dy, dz, make_float2(ff_rsqrt(r2.x), ff_rsqrt(r2.y)), s);
             }
         }
         __syncwarp();
@@ -122,16 +182,12 @@ ff_k_walk(int n, float theta, const ff_globals* __restrict__ g, const float4* __
     // append the lanes with `take` set (data A = position, B = moment) to the ring
     auto append = [&](bool take, const float4& A, const float4& B) {
         unsigned m = __ballot_sync(FF_FULL, take);
-        if (take) {
-            int slot = (pend_head + pend_cnt + __popc(m & lt)) & (FF_WALK_PEND - 1);
-            sm.pend_pos[slot] = A;
-            sm.pend_mom[slot] = B;
-        }
+        if (take) ff_ring_store(sm, (pend_head + pend_cnt + __popc(m & lt)) & (FF_WALK_PEND - 1), A, B);
         pend_cnt += __popc(m);
     };
     auto drain = [&]() {
         while (pend_cnt >= 32) {
-            eval(32);
+            eval(16);
             pend_head = (pend_head + 32) & (FF_WALK_PEND - 1);
             pend_cnt -= 32;
         }
@@ -149,7 +205,6 @@ ff_k_walk(int n, float theta, const ff_globals* __restrict__ g, const float4* __
         }
     };
 
-    const int n_cells = g->n_cells;
     if (n_cells == 0) {
         coop_leaf(0, n);                                   // the root is a leaf: plain all-pairs
     } else {
@@ -178,14 +233,21 @@ ff_k_walk(int n, float theta, const ff_globals* __restrict__ g, const float4* __
             A = __ldg(pos_s + slot); B = __ldg(mom_s + slot);
         }
         // opening test of every lane's cell against all members of the group: the group accepts iff
-        // s^2 < fl(th2 * d2_k) for every k, i.e. iff s^2 < fl(th2 * min_k d2_k) (rounding is monotone)
+        // s^2 < fl(th2 * d2_k) for every k, i.e. iff s^2 < fl(th2 * min_k d2_k) (rounding is monotone).
+        // Two members per packed instruction; d = fl(q - c) as fl(q + (-c)), d2 = fma(dz,dz,fma(dy,dy,fl(dx*dx))).
         float d2min = 3.0e38f;
+        {
+            const float2 nax = ff_dup(-A.x), nay = ff_dup(-A.y), naz = ff_dup(-A.z);
 #pragma unroll 8
-        for (int m = 0; m < 32; ++m) {
-            float4 q = sm.mem_pos[m];
-            float dx = __fsub_rn(q.x, A.x), dy = __fsub_rn(q.y, A.y), dz = __fsub_rn(q.z, A.z);
-            float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-            d2min = fminf(d2min, d2);
+            for (int m = 0; m < 16; ++m) {
+                const float4 qxy = sm.mem_xy[m];
+                const float2 qz = sm.mem_z[m];
+                const float2 dx = __fadd2_rn(make_float2(qxy.x, qxy.y), nax);
+                const float2 dy = __fadd2_rn(make_float2(qxy.z, qxy.w), nay);
+                const float2 dz = __fadd2_rn(qz, naz);
+                const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+                d2min = fminf(d2min, fminf(d2.x, d2.y));
+            }
         }
         const bool holds = first < g1 && end > g0;         // the cell's range holds a member: always open (Q3)
         const bool tested = is_cell && !holds;
@@ -230,12 +292,29 @@ ff_k_walk(int n, float theta, const ff_globals* __restrict__ g, const float4* __
         }
         __syncwarp();
     }
-    if (pend_cnt > 0) eval(pend_cnt);
+    if (pend_cnt > 0) {
+        // pad an odd tail with a copy of the last entry's position carrying a zero moment: every term
+        // of Eq. 11-12 is linear in u_j, so the pad contributes exactly 0 and stays finite
+        if (pend_cnt & 1) {
+            __syncwarp();
+            if (lane == 0) {
+                const float* f = reinterpret_cast<const float*>(sm.pend);
+                int last = (pend_head + pend_cnt - 1) & (FF_WALK_PEND - 1);
+                const float* src = f + (last >> 1) * 12 + (last & 1);
+                float4 A = make_float4(src[0], src[2], src[4], 0.f);
+                ff_ring_store(sm, (last + 1) & (FF_WALK_PEND - 1), A, make_float4(0.f, 0.f, 0.f, 0.f));
+            }
+        }
+        eval((pend_cnt + 1) >> 1);
+    }
 
     if (lane < nm) {
-        fx = fmaf(sk, ux, fx); fy = fmaf(sk, uy, fy); fz = fmaf(sk, uz, fz);
+        // fold the even / odd halves; f = fv + sk u_k
+        const float sk = s.sk.x + s.sk.y;
+        const float fx = fmaf(sk, uk.x, s.fx.x + s.fx.y), fy = fmaf(sk, uk.y, s.fy.x + s.fy.y),
+                    fz = fmaf(sk, uk.z, s.fz.x + s.fz.y);
         size_t o = (size_t)__ldg(perm + k) * 3;            // a7: back to caller order
-        if (H_out) { H_out[o] = hx; H_out[o + 1] = hy; H_out[o + 2] = hz; }
+        if (H_out) { H_out[o] = s.hx.x + s.hx.y; H_out[o + 1] = s.hy.x + s.hy.y; H_out[o + 2] = s.hz.x + s.hz.y; }
         if (F_out) { F_out[o] = fx; F_out[o + 1] = fy; F_out[o + 2] = fz; }
     }
     if (COUNT) {
@@ -247,19 +326,51 @@ ff_k_walk(int n, float theta, const ff_globals* __restrict__ g, const float4* __
     }
 }
 
+// Persistent launch: every warp fetches the next group from a device-wide counter (g->walk_next,
+// zeroed by the last cell-moment launch), so no SM idles while one block's slowest group finishes
+// and consecutive (spatially adjacent) groups run at the same time and share cells in L1/L2.
+template <bool COUNT>
+__global__ void __launch_bounds__(FF_WALK_WARPS * 32)
+ff_k_walk(int n, float theta, ff_globals* __restrict__ g, const float4* __restrict__ pos_s,
+          const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
+          const int32_t* __restrict__ cell_first,
+          const int32_t* __restrict__ cell_end, const int4* __restrict__ cell_child,
+          const int32_t* __restrict__ leaf_count, const float4* __restrict__ centre,
+          const float4* __restrict__ moment, float* __restrict__ H_out, float* __restrict__ F_out,
+          unsigned long long* __restrict__ counters)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    ff_walk_smem& sm = reinterpret_cast<ff_walk_smem*>(smem_raw)[w];
+    const int groups = (n + 31) >> 5;
+    const int n_cells = g->n_cells;
+    for (;;) {
+        int grp = 0;
+        if (lane == 0) grp = atomicAdd(&g->walk_next, 1);
+        grp = __shfl_sync(FF_FULL, grp, 0);
+        if (grp >= groups) break;
+        ff_walk_group<COUNT>(sm, grp, lane, n, theta, n_cells, pos_s, mom_s, perm, cell_first, cell_end, cell_child,
+                             leaf_count, centre, moment, H_out, F_out, counters);
+        __syncwarp();
+    }
+}
+
 int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out)
 {
     int n = (int)c->n;
     int groups = (n + 31) / 32;
-    int blocks = (groups + FF_WALK_WARPS - 1) / FF_WALK_WARPS;
     size_t smem = sizeof(ff_walk_smem) * FF_WALK_WARPS;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static int per_sm[2] = { 0, 0 };
+    if (!per_sm[0]) {
         FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
+        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], ff_k_walk<false>, FF_WALK_WARPS * 32, smem));
+        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], ff_k_walk<true>, FF_WALK_WARPS * 32, smem));
+        if (per_sm[0] < 1 || per_sm[1] < 1) return FF_ERR_CUDA;
     }
-    if (c->count_enabled) {
+    int cnt = c->count_enabled ? 1 : 0;
+    int blocks = min(c->num_sms * per_sm[cnt], (groups + FF_WALK_WARPS - 1) / FF_WALK_WARPS);
+    if (cnt) {
         FF_CUDA(c, cudaMemsetAsync(c->g->counters, 0, sizeof(c->g->counters), c->stream));
         FF_LAUNCH(c, ff_k_walk<true>, blocks, FF_WALK_WARPS * 32, smem, n, c->theta, c->g, c->pos_s, c->mom_s,
                   c->idx[0], c->cell_first, c->cell_end, (const int4*)c->cell_child,
