@@ -219,6 +219,13 @@ int ff_get_timings(ff_ctx* ctx, float ms[FF_N_PHASES]);
  */
 int ff_get_counters(ff_ctx* ctx, uint64_t* n_cell, uint64_t* n_particle, uint64_t* n_mac_tests);
 
+/*
+ * How many of the n_mac_tests of the last ff_eval_bh the walk's cheap pre-filter (group bounding box +
+ * eight probe members) could not decide and passed on to the full 32-member test
+ * (needs FF_OPT_COUNTERS).  A measurement aid: the decisions themselves are unaffected.
+ */
+int ff_get_prefilter_count(ff_ctx* ctx, uint64_t* n_parked);
+
 /* Number of kernel launches issued by this context since creation (for bench accounting). */
 int ff_get_launch_count(ff_ctx* ctx, uint64_t* launches);
 

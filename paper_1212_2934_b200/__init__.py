@@ -32,7 +32,7 @@ FF_CHILD_LEAF1, FF_CHILD_MULTI, FF_CHILD_SLOT = 0x80000000, 0x40000000, 0x3FFFFF
 SYMBOLS = (
     "ff_workspace_bytes", "ff_create", "ff_destroy", "ff_set_stream", "ff_set_option", "ff_build_tree",
     "ff_eval_bh", "ff_eval_direct", "ff_eval_bh_host", "ff_eval_direct_host", "ff_step", "ff_get_tree",
-    "ff_get_timings", "ff_get_counters", "ff_get_launch_count", "ff_measure_fp32_peak", "ff_error_string",
+    "ff_get_timings", "ff_get_counters", "ff_get_prefilter_count", "ff_get_launch_count", "ff_measure_fp32_peak", "ff_error_string",
     "ff_last_error",
 )
 
@@ -96,6 +96,8 @@ def lib():
         L.ff_get_timings.argtypes = [vp, ctypes.POINTER(f32 * FF_N_PHASES)]
         L.ff_get_counters.restype = i32
         L.ff_get_counters.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64), ctypes.POINTER(u64)]
+        L.ff_get_prefilter_count.restype = i32
+        L.ff_get_prefilter_count.argtypes = [vp, ctypes.POINTER(u64)]
         L.ff_get_launch_count.restype = i32
         L.ff_get_launch_count.argtypes = [vp, ctypes.POINTER(u64)]
         L.ff_measure_fp32_peak.restype = i32
@@ -272,6 +274,11 @@ class FFContext:
         self._check(self._L.ff_get_counters(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)),
                     "ff_get_counters")
         return int(a.value), int(b.value), int(c.value)
+
+    def prefilter_count(self) -> int:
+        a = ctypes.c_uint64()
+        self._check(self._L.ff_get_prefilter_count(self._h, ctypes.byref(a)), "ff_get_prefilter_count")
+        return int(a.value)
 
     def launch_count(self) -> int:
         a = ctypes.c_uint64()

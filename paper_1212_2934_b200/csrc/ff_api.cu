@@ -249,6 +249,16 @@ extern "C" int ff_get_counters(ff_ctx* c, uint64_t* n_cell, uint64_t* n_particle
     return FF_OK;
 }
 
+extern "C" int ff_get_prefilter_count(ff_ctx* c, uint64_t* n_parked)
+{
+    if (!c || !n_parked) return FF_ERR_INVALID_ARG;
+    FF_CUDA(c, cudaStreamSynchronize(c->stream));
+    unsigned long long v;
+    FF_CUDA(c, cudaMemcpy(&v, c->g->counters + 3, sizeof(v), cudaMemcpyDeviceToHost));
+    *n_parked = v;
+    return FF_OK;
+}
+
 extern "C" int ff_get_launch_count(ff_ctx* c, uint64_t* launches)
 {
     if (!c || !launches) return FF_ERR_INVALID_ARG;

@@ -24,9 +24,18 @@
 #define FF_SCAN_TILE (FF_SCAN_THREADS * FF_SCAN_ITEMS)
 
 // ---- walk geometry (ff_walk.cu) ---------------------------------------------
+#ifndef FF_WALK_WARPS
 #define FF_WALK_WARPS 4            // warps (= target groups) per block
+#endif
+#ifndef FF_WALK_MINB
+#define FF_WALK_MINB 1             // min resident blocks per SM asked of ptxas (register cap)
+#endif
 #define FF_WALK_STACK 1024         // traversal stack entries per warp
 #define FF_WALK_PEND 64            // pending interaction ring per warp (two batches of 32)
+#ifndef FF_WALK_PROBE_PAIRS
+#define FF_WALK_PROBE_PAIRS 2      // probe members (x2) of the opening pre-filter, taken in the order: the members
+#endif                             // at the x, y, z extremes of the group's box, then the first and the last member
+#define FF_WALK_AMB_ROOM 256       // stack room an ambiguous-queue round may need (32 cells x 8 children)
 
 // ---- direct geometry (ff_direct.cu) -------------------------------------------
 #define FF_DIRECT_THREADS 256
@@ -42,7 +51,7 @@ struct ff_globals {
     int32_t n_cells;          // internal cells of the current tree
     int32_t error;            // sticky device-side error flag (FF_ERR_*)
     int32_t walk_next;        // next target group of the persistent walk (zeroed by the level-0 moment launch)
-    unsigned long long counters[3];   // n_cell, n_particle, n_mac (FF_OPT_COUNTERS)
+    unsigned long long counters[4];   // n_cell, n_particle, n_mac, n_parked (FF_OPT_COUNTERS)
     uint32_t digit_total[FF_RADIX];   // per-pass digit totals (ff_sort.cu)
 };
 

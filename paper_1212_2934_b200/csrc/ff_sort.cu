@@ -13,7 +13,7 @@ __global__ void ff_k_reset(ff_globals* g)
 {
     int t = threadIdx.x;
     if (t < 3) { g->bbox_ord[t] = 0xffffffffu; g->bbox_ord[4 + t] = 0u; }
-    if (t < 3) g->counters[t] = 0ull;
+    if (t < 4) g->counters[t] = 0ull;
     if (t == 0) g->n_cells = 0;
 }
 

@@ -35,6 +35,10 @@ struct ff_walk_smem {
     float4 pend[FF_PEND_PAIRS * 3];    // pair p: [3p] = x0,x1,y0,y1  [3p+1] = z0,z1,mx0,mx1  [3p+2] = my0,my1,mz0,mz1
     float4 mem_xy[16];                 // group members, pair m: x0,x1,y0,y1
     float2 mem_z[16];                  //                        z0,z1
+    float4 probe_xy[FF_WALK_PROBE_PAIRS];   // probe members of the opening pre-filter, same pair layout
+    float2 probe_z[FF_WALK_PROBE_PAIRS];
+    float4 bb_lo, bb_hi;               // bounding box of the group's members (exact min / max)
+    int32_t amb[64];                   // cells the pre-filter could not decide, waiting for the full test
 };
 
 __device__ __forceinline__ float2 ff_dup(float a) { return make_float2(a, a); }
@@ -129,13 +133,37 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
     tg.ux = ff_dup(uk.x); tg.uy = ff_dup(uk.y); tg.uz = ff_dup(uk.z);
     ff_acc2 s;
     s.hx = s.hy = s.hz = s.fx = s.fy = s.fz = s.sk = ff_dup(0.0f);
-    unsigned long long c_cell = 0, c_part = 0, c_mac = 0;
+    unsigned long long c_cell = 0, c_part = 0, c_mac = 0, c_amb = 0;
 
     {   // group members in pair layout for the opening test; the ring's first batch = the members themselves
         float* mxy = reinterpret_cast<float*>(sm.mem_xy) + (lane >> 1) * 4 + (lane & 1);
         mxy[0] = pk.x; mxy[2] = pk.y;
         reinterpret_cast<float*>(sm.mem_z)[lane] = pk.z;
         ff_ring_store(sm, lane, pk, uk);
+        // pre-filter data: exact bounding box of the members and the probe members (the members that
+        // attain the box extremes -- chosen on a key that trades the 5 low bits for the lane --, the
+        // first and the last).  Lanes past a ragged end hold copies of the last member, which is harmless.
+        const uint32_t ox = ff_f2ord(pk.x), oy = ff_f2ord(pk.y), oz = ff_f2ord(pk.z);
+        const float lox = ff_ord2f(__reduce_min_sync(FF_FULL, ox)), hix = ff_ord2f(__reduce_max_sync(FF_FULL, ox));
+        const float loy = ff_ord2f(__reduce_min_sync(FF_FULL, oy)), hiy = ff_ord2f(__reduce_max_sync(FF_FULL, oy));
+        const float loz = ff_ord2f(__reduce_min_sync(FF_FULL, oz)), hiz = ff_ord2f(__reduce_max_sync(FF_FULL, oz));
+        if (lane == 0) {
+            sm.bb_lo = make_float4(lox, loy, loz, 0.f);
+            sm.bb_hi = make_float4(hix, hiy, hiz, 0.f);
+        }
+        const uint32_t kx = (ox & ~31u) | lane, ky = (oy & ~31u) | lane, kz = (oz & ~31u) | lane;
+        int src[8];
+        src[0] = __reduce_min_sync(FF_FULL, kx) & 31; src[1] = __reduce_max_sync(FF_FULL, kx) & 31;
+        src[2] = __reduce_min_sync(FF_FULL, ky) & 31; src[3] = __reduce_max_sync(FF_FULL, ky) & 31;
+        src[4] = __reduce_min_sync(FF_FULL, kz) & 31; src[5] = __reduce_max_sync(FF_FULL, kz) & 31;
+        src[6] = 0; src[7] = 31;
+#pragma unroll
+        for (int t = 0; t < 2 * FF_WALK_PROBE_PAIRS; ++t)
+            if (lane == src[t]) {
+                float* f = reinterpret_cast<float*>(sm.probe_xy) + (t >> 1) * 4 + (t & 1);
+                f[0] = pk.x; f[2] = pk.y;
+                reinterpret_cast<float*>(sm.probe_z)[t] = pk.z;
+            }
     }
     __syncwarp();
     // the group's own members: direct terms, self skipped by index (Alg. 1 line 5);
@@ -213,12 +241,26 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
         __syncwarp();
     }
 
-    while (sp_top > 0) {
-        // entries popped this round; bounded so that the pushes always fit (walk stack)
-        int room = FF_WALK_STACK - 80 - sp_top;
-        int p = min(sp_top, max(1, min(32, room / 7)));
-        int32_t e = (lane < p) ? sm.stack[sp_top - 1 - lane] : FF_CHILD_EMPTY;
-        sp_top -= p;
+    int amb_cnt = 0;                                       // warp-uniform size of the ambiguous queue
+    while (sp_top > 0 || amb_cnt > 0) {
+        // Source of this round's entries.  Normal round: pop the stack, decide cells with the cheap
+        // pre-filter, park the undecided ones in sm.amb.  Ambiguous round (32 parked, or the stack ran
+        // dry): full 32-member test on parked cells.  Stack nearly full: pop one entry at a time as
+        // before; parked cells wait (and, if 32 are parked already, popped cells get the full test).
+        const int room = FF_WALK_STACK - 80 - sp_top;
+        const bool amb_round = sp_top == 0 || (amb_cnt >= 32 && room >= FF_WALK_AMB_ROOM);
+        const bool full = amb_round || amb_cnt >= 32;
+        int32_t e;
+        if (amb_round) {
+            const int p = min(amb_cnt, 32);
+            e = (lane < p) ? sm.amb[amb_cnt - 1 - lane] : FF_CHILD_EMPTY;
+            amb_cnt -= p;
+        } else {
+            // entries popped this round; bounded so that the pushes always fit (walk stack)
+            const int p = min(sp_top, max(1, min(32, room / 7)));
+            e = (lane < p) ? sm.stack[sp_top - 1 - lane] : FF_CHILD_EMPTY;
+            sp_top -= p;
+        }
         __syncwarp();
         const bool is_cell = e >= 0;
         const bool is_part = !is_cell && e != FF_CHILD_EMPTY && !((uint32_t)e & FF_CHILD_MULTI);
@@ -228,16 +270,17 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
         int first = 0, end = 0;
         if (is_cell) {
             A = __ldg(centre + e); B = __ldg(moment + e);
-            first = __ldg(cell_first + e); end = __ldg(cell_end + e);
+            if (!amb_round) { first = __ldg(cell_first + e); end = __ldg(cell_end + e); }
         } else if (is_part) {
             A = __ldg(pos_s + slot); B = __ldg(mom_s + slot);
         }
-        // opening test of every lane's cell against all members of the group: the group accepts iff
-        // s^2 < fl(th2 * d2_k) for every k, i.e. iff s^2 < fl(th2 * min_k d2_k) (rounding is monotone).
-        // Two members per packed instruction; d = fl(q - c) as fl(q + (-c)), d2 = fma(dz,dz,fma(dy,dy,fl(dx*dx))).
-        float d2min = 3.0e38f;
-        {
-            const float2 nax = ff_dup(-A.x), nay = ff_dup(-A.y), naz = ff_dup(-A.z);
+        // Opening rule O5: the group accepts a cell iff s^2 < fl(th2 * d2_k) for every member k, i.e. iff
+        // s^2 < fl(th2 * min_k d2_k) (rounding is monotone), with d = fl(q - c) as fl(q + (-c)) and
+        // d2 = fma(dz,dz,fma(dy,dy,fl(dx*dx))); two members per packed instruction.
+        bool acc, amb = false;
+        const float2 nax = ff_dup(-A.x), nay = ff_dup(-A.y), naz = ff_dup(-A.z);
+        if (full) {
+            float d2min = 3.0e38f;
 #pragma unroll 8
             for (int m = 0; m < 16; ++m) {
                 const float4 qxy = sm.mem_xy[m];
@@ -248,16 +291,48 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
                 const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
                 d2min = fminf(d2min, fminf(d2.x, d2.y));
             }
+            acc = A.w < __fmul_rn(th2, d2min);
+        } else {
+            // Pre-filter.  (1) Sure accept: every member lies in the box, so per axis |q - c| >= e_a =
+            // max(lo_a - c_a, c_a - hi_a, 0) and every exact d2_k >= e.e; the fp32 values of both sides
+            // are within 6 ulp of their exact ones and the products within 1, so a margin of 2^-19
+            // (0.999998f) makes "s^2 < th2 * e.e * margin" imply the exact test of every member.
+            // (2) Sure open: the exact test of a probe member fails.  Anything else is parked.
+            const float4 lo = sm.bb_lo, hi = sm.bb_hi;
+            const float ex = fmaxf(fmaxf(lo.x - A.x, A.x - hi.x), 0.f);
+            const float ey = fmaxf(fmaxf(lo.y - A.y, A.y - hi.y), 0.f);
+            const float ez = fmaxf(fmaxf(lo.z - A.z, A.z - hi.z), 0.f);
+            const float e2 = fmaf(ez, ez, fmaf(ey, ey, ex * ex));
+            acc = A.w < th2 * e2 * 0.999998f;
+            float d2min = 3.0e38f;
+#pragma unroll
+            for (int m = 0; m < FF_WALK_PROBE_PAIRS; ++m) {
+                const float4 qxy = sm.probe_xy[m];
+                const float2 qz = sm.probe_z[m];
+                const float2 dx = __fadd2_rn(make_float2(qxy.x, qxy.y), nax);
+                const float2 dy = __fadd2_rn(make_float2(qxy.z, qxy.w), nay);
+                const float2 dz = __fadd2_rn(qz, naz);
+                const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+                d2min = fminf(d2min, fminf(d2.x, d2.y));
+            }
+            amb = !acc && (A.w < __fmul_rn(th2, d2min));
         }
         const bool holds = first < g1 && end > g0;         // the cell's range holds a member: always open (Q3)
         const bool tested = is_cell && !holds;
-        const bool accept_cell = tested && (A.w < __fmul_rn(th2, d2min));
-        const bool open = is_cell && !accept_cell;
+        const bool accept_cell = tested && acc;
+        const bool park = tested && amb;
+        const bool open = is_cell && !accept_cell && !park;
         const bool take = accept_cell || (is_part && !(slot >= g0 && slot < g1));
         if (COUNT) {
-            c_mac += __popc(__ballot_sync(FF_FULL, tested));
+            c_mac += __popc(__ballot_sync(FF_FULL, tested && !amb_round));
             c_cell += (unsigned long long)__popc(__ballot_sync(FF_FULL, accept_cell)) * nm;
             c_part += (unsigned long long)__popc(__ballot_sync(FF_FULL, take && is_part)) * nm;
+            c_amb += __popc(__ballot_sync(FF_FULL, park));
+        }
+        if (!full) {
+            const unsigned pm = __ballot_sync(FF_FULL, park);
+            if (park) sm.amb[amb_cnt + __popc(pm & lt)] = e;
+            amb_cnt += __popc(pm);
         }
         append(take, A, B);
         int4 c0 = make_int4(-1, -1, -1, -1), c1 = c0;
@@ -322,6 +397,7 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
             atomicAdd(counters + 0, c_cell);
             atomicAdd(counters + 1, c_part);
             atomicAdd(counters + 2, c_mac);
+            atomicAdd(counters + 3, c_amb);
         }
     }
 }
@@ -330,7 +406,7 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
 // zeroed by the last cell-moment launch), so no SM idles while one block's slowest group finishes
 // and consecutive (spatially adjacent) groups run at the same time and share cells in L1/L2.
 template <bool COUNT>
-__global__ void __launch_bounds__(FF_WALK_WARPS * 32)
+__global__ void __launch_bounds__(FF_WALK_WARPS * 32, FF_WALK_MINB)
 ff_k_walk(int n, float theta, ff_globals* __restrict__ g, const float4* __restrict__ pos_s,
           const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
           const int32_t* __restrict__ cell_first,
