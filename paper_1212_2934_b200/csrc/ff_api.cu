@@ -140,8 +140,7 @@ extern "C" int ff_eval_bh(ff_ctx* c, const float* pos, const float* mom, float* 
     if (!c->tree_built) return FF_ERR_NO_TREE;
     int rc;
     ff_phase_begin(c, FF_PH_MOMENTS);
-    if ((rc = ff_launch_gather_mom(c, mom)) != FF_OK) return rc;
-    if ((rc = ff_launch_moments(c)) != FF_OK) return rc;
+    if ((rc = ff_launch_moments(c, mom)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_MOMENTS);
     c->moments_valid = 1;
     ff_phase_begin(c, FF_PH_WALK);

@@ -14,6 +14,10 @@
 // An exclusive scan of that count numbers the cells in pre-order, i.e. sorted by
 // (first, level).  Children and ranges come from binary searches in the key array.
 #include "ff_internal.cuh"
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
+
+#define FF_MOM_THREADS 256
 
 __device__ __forceinline__ int ff_lprev(const uint32_t* __restrict__ key, int i)
 {
@@ -126,6 +130,10 @@ ff_k_cells_fill(const uint32_t* __restrict__ key, int n, int nleaf, const int32_
     if (i >= n) return;
     int lprev;
     int cnt = ff_cells_at(key, i, n, nleaf, lprev);
+    {   // deepest level holding an internal cell (bounds the level loop of ff_k_moments)
+        int deepest = __reduce_max_sync(__activemask(), cnt > 0 ? lprev + cnt : 0);
+        if (ff_lane() == 0 && deepest > 0) atomicMax(&g->max_level, deepest);
+    }
     if (cnt == 0) return;
     int base = cell_base[i];
     if (base + cnt > cell_cap) { g->error = FF_ERR_CAPACITY; return; }
@@ -166,56 +174,84 @@ ff_k_cells_fill(const uint32_t* __restrict__ key, int n, int nleaf, const int32_
     }
 }
 
-// ---- a5: Eq. 14, one level per launch, deepest first ------------
+// ---- a5: Eq. 14: ONE cooperative launch -----------------------
+// Phase 0 gathers the moments into sorted float4 order; then the levels are summed deepest
+// first with a grid-wide barrier between levels (the paper's kernel 3 lets threads spin on
+// their children instead; ten launches cost ~14 us each at N = 2^20).
 // fp64 sums in the fixed order of DESIGN.md (O4): children in octant order,
 // ((c0 + c1) + c2) + ...; a leaf's particles left to right; one fp64 divide and a
 // single rounding to fp32.
-__global__ void __launch_bounds__(128)
-ff_k_moments_level(int level, ff_globals* __restrict__ g, const int32_t* __restrict__ cell_first,
-                   const int32_t* __restrict__ cell_end, const int32_t* __restrict__ cell_level,
-                   const int32_t* __restrict__ cell_child, const int32_t* __restrict__ leaf_count,
-                   const float4* __restrict__ pos_s, const float4* __restrict__ mom_s,
-                   double* __restrict__ sum_u, double* __restrict__ sum_p,
-                   float4* __restrict__ centre, float4* __restrict__ moment)
+__global__ void __launch_bounds__(FF_MOM_THREADS)
+ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, int n, ff_globals* __restrict__ g,
+             const int32_t* __restrict__ cell_first, const int32_t* __restrict__ cell_end,
+             const int32_t* __restrict__ cell_level, const int32_t* __restrict__ cell_child,
+             const int32_t* __restrict__ leaf_count, const float4* __restrict__ pos_s, float4* __restrict__ mom_s,
+             double* __restrict__ sum_u, double* __restrict__ sum_p, float4* __restrict__ centre,
+             float4* __restrict__ moment)
 {
-    int n_cells = g->n_cells;
-    if (level == 0 && blockIdx.x == 0 && threadIdx.x == 0) g->walk_next = 0;   // last launch before the walk
-    float s = ldexpf(g->S, -level);
-    float s2 = __fmul_rn(s, s);
-    for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < n_cells; id += gridDim.x * blockDim.x) {
-        if (cell_level[id] != level) continue;
-        double su[3], sp[3];
-        bool started = false;
-        for (int o = 0; o < 8; ++o) {
-            int32_t e = cell_child[8 * (size_t)id + o];
-            if (e == FF_CHILD_EMPTY) continue;
-            double cu[3], cp[3];
+    cg::grid_group grid = cg::this_grid();
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    for (int s = tid; s < n; s += nth) {
+        size_t j = (size_t)__ldg(perm + s) * 3;
+        mom_s[s] = make_float4(__ldg(mom + j), __ldg(mom + j + 1), __ldg(mom + j + 2), 0.0f);
+    }
+    if (tid == 0) g->walk_next = 0;                        // the walk's group counter (this is the last launch before it)
+    const int n_cells = g->n_cells;
+    const int top = min(g->max_level, FF_MAX_LEVEL - 1);   // deepest level that holds an internal cell
+    const float S = g->S;
+    // Eight lanes per cell: lane o loads child o (one exposed memory latency per cell instead of eight),
+    // parks its six fp64 sums in shared memory, then lane a < 6 adds component a over the children in
+    // octant order -- the same ((c0 + c1) + c2) + ... as a sequential loop.
+    __shared__ double sh[FF_MOM_THREADS / 8][8][6];
+    const int o = threadIdx.x & 7;
+    const unsigned gshift = (threadIdx.x & 24);            // first lane of this group inside the warp
+    const unsigned gmask = 0xffu << gshift;
+    double(*mine)[6] = sh[threadIdx.x >> 3];
+    const int gid = tid >> 3, ngroups = nth >> 3;
+    grid.sync();
+    for (int level = top; level >= 0; --level) {
+        const float s = ldexpf(S, -level);
+        const float s2 = __fmul_rn(s, s);
+        for (int id = gid; id < n_cells; id += ngroups) {
+            if (cell_level[id] != level) continue;         // uniform over the group's eight lanes
+            const int32_t e = cell_child[8 * (size_t)id + o];
+            const bool have = e != FF_CHILD_EMPTY;
             if (e >= 0) {
+                // plain loads: written earlier in this launch by other blocks (ordered by grid.sync)
 #pragma unroll
-                for (int a = 0; a < 3; ++a) { cu[a] = sum_u[3 * (size_t)e + a]; cp[a] = sum_p[3 * (size_t)e + a]; }
-            } else {
+                for (int a = 0; a < 3; ++a) { mine[o][a] = sum_u[3 * (size_t)e + a]; mine[o][3 + a] = sum_p[3 * (size_t)e + a]; }
+            } else if (have) {
                 int slot = (int)((uint32_t)e & FF_CHILD_SLOT);
                 int cc = ((uint32_t)e & FF_CHILD_MULTI) ? leaf_count[slot] : 1;
                 float4 p = pos_s[slot], m = mom_s[slot];
-                cu[0] = m.x; cu[1] = m.y; cu[2] = m.z;
-                cp[0] = p.x; cp[1] = p.y; cp[2] = p.z;
+                double cu[3] = { m.x, m.y, m.z }, cp[3] = { p.x, p.y, p.z };
                 for (int j = slot + 1; j < slot + cc; ++j) {
                     p = pos_s[j]; m = mom_s[j];
                     cu[0] += (double)m.x; cu[1] += (double)m.y; cu[2] += (double)m.z;
                     cp[0] += (double)p.x; cp[1] += (double)p.y; cp[2] += (double)p.z;
                 }
-            }
 #pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                if (!started) { su[a] = cu[a]; sp[a] = cp[a]; } else { su[a] += cu[a]; sp[a] += cp[a]; }
+                for (int a = 0; a < 3; ++a) { mine[o][a] = cu[a]; mine[o][3 + a] = cp[a]; }
             }
-            started = true;
+            const unsigned present = (__ballot_sync(gmask, have) >> gshift) & 0xffu;   // also orders the smem writes
+            const double cnt = (double)(cell_end[id] - cell_first[id]);
+            double t = 0.0;
+            if (o < 6) {
+                bool started = false;
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    if (present & (1u << c)) { t = started ? t + mine[c][o] : mine[c][o]; started = true; }
+                if (o < 3) sum_u[3 * (size_t)id + o] = t; else sum_p[3 * (size_t)id + (o - 3)] = t;
+            }
+            float* cen = reinterpret_cast<float*>(centre + id);
+            float* mo = reinterpret_cast<float*>(moment + id);
+            if (o < 3) mo[o] = (float)t;
+            else if (o < 6) cen[o - 3] = (float)(t / cnt);
+            else if (o == 6) cen[3] = s2;
+            else mo[3] = (float)cnt;
+            __syncwarp(gmask);                             // smem slots are reused by the group's next cell
         }
-        double cnt = (double)(cell_end[id] - cell_first[id]);
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { sum_u[3 * (size_t)id + a] = su[a]; sum_p[3 * (size_t)id + a] = sp[a]; }
-        centre[id] = make_float4((float)(sp[0] / cnt), (float)(sp[1] / cnt), (float)(sp[2] / cnt), s2);
-        moment[id] = make_float4((float)su[0], (float)su[1], (float)su[2], (float)cnt);
+        if (level > 0) grid.sync();
     }
 }
 
@@ -231,13 +267,22 @@ int ff_launch_build(ff_ctx* c)
     return FF_OK;
 }
 
-int ff_launch_moments(ff_ctx* c)
+int ff_launch_moments(ff_ctx* c, const float* mom)
 {
     int n = (int)c->n;
-    int blocks = min((n + 127) / 128, c->num_sms * 16);
-    for (int level = FF_MAX_LEVEL - 1; level >= 0; --level)
-        FF_LAUNCH(c, ff_k_moments_level, blocks, 128, 0, level, c->g, c->cell_first, c->cell_end, c->cell_level,
-                  c->cell_child, c->leaf_count, c->pos_s, c->mom_s, c->cell_sum_u, c->cell_sum_p, c->cell_centre,
-                  c->cell_moment);
+    static int per_sm = 0;
+    if (!per_sm) {
+        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_moments, FF_MOM_THREADS, 0));
+        if (per_sm < 1) return FF_ERR_CUDA;
+    }
+    int blocks = min((n + FF_MOM_THREADS - 1) / FF_MOM_THREADS, c->num_sms * min(per_sm, 8));
+    const uint32_t* perm = c->idx[0];
+    void* args[] = { (void*)&mom, (void*)&perm, (void*)&n, (void*)&c->g, (void*)&c->cell_first, (void*)&c->cell_end,
+                     (void*)&c->cell_level, (void*)&c->cell_child, (void*)&c->leaf_count, (void*)&c->pos_s,
+                     (void*)&c->mom_s, (void*)&c->cell_sum_u, (void*)&c->cell_sum_p, (void*)&c->cell_centre,
+                     (void*)&c->cell_moment };
+    FF_CUDA(c, cudaLaunchCooperativeKernel((const void*)ff_k_moments, dim3(blocks), dim3(FF_MOM_THREADS), args, 0,
+                                           c->stream));
+    c->launches++;
     return FF_OK;
 }

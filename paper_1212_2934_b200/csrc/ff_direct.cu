@@ -8,83 +8,79 @@
 // sums so that 10^6 sources keep 1e-5 relative accuracy; small N is split over
 // source chunks so the grid still covers all 148 SMs.
 #include "ff_internal.cuh"
+#include "ff_pair.cuh"
 
-__device__ __forceinline__ void ff_pair_accum_d(float dx, float dy, float dz, float rinv, float ux, float uy, float uz,
-                                                float mx, float my, float mz, float& hx, float& hy, float& hz,
-                                                float& fx, float& fy, float& fz, float& sk)
+// MUFU.RSQ + one Newton step, two sources at a time: the all-pairs tolerance is 1e-5 on sums
+// dominated by a few near terms, and r^-5 amplifies the 1-2 ulp of the raw approximation five times
+__device__ __forceinline__ float2 ff_rsqrt2_nr(float2 r2)
 {
-    float rinv2 = rinv * rinv;
-    float rinv3 = rinv2 * rinv;
-    float r5x3 = 3.0f * (rinv3 * rinv2);
-    float a = fmaf(mz, dz, fmaf(my, dy, mx * dx));
-    float b = fmaf(uz, dz, fmaf(uy, dy, ux * dx));
-    float cc = fmaf(mz, uz, fmaf(my, uy, mx * ux));
-    float ca = a * r5x3;
-    float cb = b * r5x3;
-    hx = fmaf(ca, dx, hx); hy = fmaf(ca, dy, hy); hz = fmaf(ca, dz, hz);
-    hx = fmaf(-rinv3, mx, hx); hy = fmaf(-rinv3, my, hy); hz = fmaf(-rinv3, mz, hz);
-    float t = (a * b) * rinv2;
-    float cr = fmaf(-5.0f, t, cc) * r5x3;
-    fx = fmaf(cr, dx, fx); fy = fmaf(cr, dy, fy); fz = fmaf(cr, dz, fz);
-    fx = fmaf(cb, mx, fx); fy = fmaf(cb, my, fy); fz = fmaf(cb, mz, fz);
-    sk += ca;
+    const float2 y = make_float2(ff_rsqrt(r2.x), ff_rsqrt(r2.y));
+    const float2 t = __fmul2_rn(r2, y);
+    const float2 e = __ffma2_rn(t, make_float2(-y.x, -y.y), ff_dup(1.0f));      // 1 - r2 y^2
+    return __ffma2_rn(__fmul2_rn(y, ff_dup(0.5f)), e, y);                       // y (1 + e/2)
 }
 
-// rsqrt with one Newton step: the all-pairs tolerance is 1e-5 on sums dominated by a few near terms
-__device__ __forceinline__ float ff_rsqrt_nr(float r2)
-{
-    float y = rsqrtf(r2);
-    return y * fmaf(-0.5f * r2, y * y, 1.5f);
-}
+#define FF_DIRECT_PAIRS (FF_DIRECT_THREADS / 2)
 
 // grid = (target blocks, source splits).  Block (bx, by) accumulates, for its 256 targets, the
-// sources of tiles by, by + splits, by + 2 splits, ...
+// sources of tiles by, by + splits, by + 2 splits, ...  A tile is staged in shared memory in the pair
+// layout of ff_pair.cuh, so that one lane evaluates two sources per packed instruction.
 __global__ void __launch_bounds__(FF_DIRECT_THREADS)
 ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n, int splits,
             double* __restrict__ part, float* __restrict__ H_out, float* __restrict__ F_out)
 {
-    __shared__ float4 spos[FF_DIRECT_THREADS], smom[FF_DIRECT_THREADS];
+    __shared__ float4 tile_q[FF_DIRECT_PAIRS * 3];
     const int t = threadIdx.x;
     const int k = blockIdx.x * FF_DIRECT_THREADS + t;
     const int kk = min(k, n - 1);
-    const float px = __ldg(pos + 3 * (size_t)kk), py = __ldg(pos + 3 * (size_t)kk + 1), pz = __ldg(pos + 3 * (size_t)kk + 2);
     const float ux = __ldg(mom + 3 * (size_t)kk), uy = __ldg(mom + 3 * (size_t)kk + 1), uz = __ldg(mom + 3 * (size_t)kk + 2);
+    ff_target2 tg;
+    tg.px = ff_dup(__ldg(pos + 3 * (size_t)kk)); tg.py = ff_dup(__ldg(pos + 3 * (size_t)kk + 1));
+    tg.pz = ff_dup(__ldg(pos + 3 * (size_t)kk + 2));
+    tg.ux = ff_dup(ux); tg.uy = ff_dup(uy); tg.uz = ff_dup(uz);
     double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };
     const int n_tiles = (n + FF_DIRECT_THREADS - 1) / FF_DIRECT_THREADS;
+    float* mine = reinterpret_cast<float*>(tile_q) + (t >> 1) * 12 + (t & 1);
     for (int tile = blockIdx.y; tile < n_tiles; tile += splits) {
         int j = tile * FF_DIRECT_THREADS + t;
-        float4 sp = make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.f), sv = make_float4(0.f, 0.f, 0.f, 0.f);   // padding: zero moment, far away
+        float sx = 3.0e18f, sy = 3.0e18f, sz = 3.0e18f, vx = 0.f, vy = 0.f, vz = 0.f;   // padding: zero moment, far away
         if (j < n) {
-            sp = make_float4(__ldg(pos + 3 * (size_t)j), __ldg(pos + 3 * (size_t)j + 1), __ldg(pos + 3 * (size_t)j + 2), 0.f);
-            sv = make_float4(__ldg(mom + 3 * (size_t)j), __ldg(mom + 3 * (size_t)j + 1), __ldg(mom + 3 * (size_t)j + 2), 0.f);
+            sx = __ldg(pos + 3 * (size_t)j); sy = __ldg(pos + 3 * (size_t)j + 1); sz = __ldg(pos + 3 * (size_t)j + 2);
+            vx = __ldg(mom + 3 * (size_t)j); vy = __ldg(mom + 3 * (size_t)j + 1); vz = __ldg(mom + 3 * (size_t)j + 2);
         }
         __syncthreads();
-        spos[t] = sp; smom[t] = sv;
+        mine[0] = sx; mine[2] = sy; mine[4] = sz; mine[6] = vx; mine[8] = vy; mine[10] = vz;
         __syncthreads();
         // fp32 partial sums over chunks of 32 sources, folded into the fp64 running sums: keeps the
         // accumulation error at sqrt(32) ulp of a chunk sum instead of sqrt(N) ulp of the total
         const bool own = tile == blockIdx.x;     // the only tile that holds this block's own targets
-        for (int c0 = 0; c0 < FF_DIRECT_THREADS; c0 += 32) {
-            float hx = 0.f, hy = 0.f, hz = 0.f, fx = 0.f, fy = 0.f, fz = 0.f, sk = 0.f;
+        for (int c0 = 0; c0 < FF_DIRECT_PAIRS; c0 += 16) {
+            ff_acc2 s;
+            s.hx = s.hy = s.hz = s.fx = s.fy = s.fz = s.sk = ff_dup(0.0f);
+            const float4* q = tile_q + 3 * c0;
             if (own) {
-#pragma unroll 4
-                for (int i = c0; i < c0 + 32; ++i) {
-                    float4 a = spos[i], m = smom[i];
-                    float dx = px - a.x, dy = py - a.y, dz = pz - a.z;
-                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    float rinv = (i == t) ? 0.0f : ff_rsqrt_nr(r2);   // j + i != k (Alg. 1 line 5)
-                    ff_pair_accum_d(dx, dy, dz, rinv, ux, uy, uz, m.x, m.y, m.z, hx, hy, hz, fx, fy, fz, sk);
+#pragma unroll 2
+                for (int i = 0; i < 16; ++i) {
+                    const float4 q0 = q[3 * i], q1 = q[3 * i + 1], q2 = q[3 * i + 2];
+                    float2 dx, dy, dz, r2;
+                    ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
+                    float2 rinv = ff_rsqrt2_nr(r2);
+                    if (2 * (c0 + i) == t) rinv.x = 0.0f;          // j != k (Alg. 1 line 5): r2 = 0 gave NaN, dropped here
+                    if (2 * (c0 + i) + 1 == t) rinv.y = 0.0f;
+                    ff_pair2_accum(q1, q2, tg, dx, dy, dz, rinv, s);
                 }
             } else {
-#pragma unroll 8
-                for (int i = c0; i < c0 + 32; ++i) {
-                    float4 a = spos[i], m = smom[i];
-                    float dx = px - a.x, dy = py - a.y, dz = pz - a.z;
-                    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    ff_pair_accum_d(dx, dy, dz, ff_rsqrt_nr(r2), ux, uy, uz, m.x, m.y, m.z, hx, hy, hz, fx, fy, fz, sk);
+#pragma unroll 4
+                for (int i = 0; i < 16; ++i) {
+                    const float4 q0 = q[3 * i], q1 = q[3 * i + 1], q2 = q[3 * i + 2];
+                    float2 dx, dy, dz, r2;
+                    ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
+                    ff_pair2_accum(q1, q2, tg, dx, dy, dz, ff_rsqrt2_nr(r2), s);
                 }
             }
-            acc[0] += hx; acc[1] += hy; acc[2] += hz; acc[3] += fx; acc[4] += fy; acc[5] += fz; acc[6] += sk;
+            acc[0] += s.hx.x + s.hx.y; acc[1] += s.hy.x + s.hy.y; acc[2] += s.hz.x + s.hz.y;
+            acc[3] += s.fx.x + s.fx.y; acc[4] += s.fy.x + s.fy.y; acc[5] += s.fz.x + s.fz.y;
+            acc[6] += s.sk.x + s.sk.y;
         }
     }
     if (k >= n) return;

@@ -50,6 +50,7 @@ struct ff_globals {
     float inv;                // fl(1024 / S)
     int32_t n_cells;          // internal cells of the current tree
     int32_t error;            // sticky device-side error flag (FF_ERR_*)
+    int32_t max_level;        // deepest level holding an internal cell (atomicMax in ff_k_cells_fill)
     int32_t walk_next;        // next target group of the persistent walk (zeroed by the level-0 moment launch)
     unsigned long long counters[4];   // n_cell, n_particle, n_mac, n_parked (FF_OPT_COUNTERS)
     uint32_t digit_total[FF_RADIX];   // per-pass digit totals (ff_sort.cu)
@@ -127,8 +128,7 @@ static inline void ff_phase_end(ff_ctx* c, int ph)
 int ff_launch_bbox_keys(ff_ctx* c, const float* pos);
 int ff_launch_sort(ff_ctx* c, const float* pos);
 int ff_launch_build(ff_ctx* c);
-int ff_launch_gather_mom(ff_ctx* c, const float* mom);
-int ff_launch_moments(ff_ctx* c);
+int ff_launch_moments(ff_ctx* c, const float* mom);
 int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out);
 int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n, float* H_out, float* F_out);
 int ff_launch_fp32_peak(ff_ctx* c, int iters, double* tflops);

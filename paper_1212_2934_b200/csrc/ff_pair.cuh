@@ -1,0 +1,69 @@
+// ff_pair.cuh -- Eq. 11 (field) and Eq. 12 (force) pair terms in packed FP32.
+//
+// sm_100 has packed FP32 instructions (FFMA2 / FMUL2 / FADD2, reached through __ffma2_rn,
+// __fmul2_rn, __fadd2_rn): one lane handles TWO sources per instruction.  The FP32 pipe does the
+// same work but needs half the issue slots.  Sources therefore come in PAIRS of three float4:
+//   q0 = x0,x1,y0,y1   q1 = z0,z1,mx0,mx1   q2 = my0,my1,mz0,mz1
+// Used by the tree walk (ff_walk.cu) and by the tiled all-pairs kernel (ff_direct.cu).
+#pragma once
+#include <cuda_runtime.h>
+
+__device__ __forceinline__ float2 ff_dup(float a) { return make_float2(a, a); }
+
+// MUFU.RSQ without the denormal pre/post-scaling of rsqrtf (2 FSETP + 4 FMUL per pair of sources):
+// r^2 of two distinct particles is never denormal for inputs the ABI allows.
+__device__ __forceinline__ float ff_rsqrt(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// target-side registers of one lane: position and moment duplicated into both halves of a pair
+struct ff_target2 {
+    float2 px, py, pz, ux, uy, uz;
+};
+
+// running sums of one lane, even / odd sources in the two halves; f = fv + sk u_k (the u_k term
+// of Eq. 12 is accumulated as a scalar and applied once at the end).  The two parts of Eq. 11 go
+// into ONE accumulator: for aligned moments sum 3 rho (u.rho)/r^5 and sum u/r^3 are each far larger
+// than their difference, and separate fp32 sums would lose that difference to rounding.
+struct ff_acc2 {
+    float2 hx, hy, hz, fx, fy, fz, sk;
+};
+
+// Two source terms of Eq. 11 (h) and Eq. 12 (f) for one target.  q0,q1,q2 = the pair's three
+// float4 of the ring; rinv = 1/|rho| per half (0 for a term that is to be skipped).
+//   h_kj = 3 rho (u_j.rho)/r^5 - u_j/r^3
+//   f_kj = { rho [(u_j.u_k) - 5 (u_j.rho)(u_k.rho)/r^2] + u_k (u_j.rho) + u_j (u_k.rho) } 3/r^5
+__device__ __forceinline__ void ff_pair2_geom(const float4& q0, const float4& q1, const ff_target2& t, float2& dx,
+                                              float2& dy, float2& dz, float2& r2)
+{
+    const float2 neg1 = ff_dup(-1.0f);
+    dx = __ffma2_rn(make_float2(q0.x, q0.y), neg1, t.px);    // rho = p_k - p_j (one rounding, as a subtraction)
+    dy = __ffma2_rn(make_float2(q0.z, q0.w), neg1, t.py);
+    dz = __ffma2_rn(make_float2(q1.x, q1.y), neg1, t.pz);
+    r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+}
+
+__device__ __forceinline__ void ff_pair2_accum(const float4& q1, const float4& q2, const ff_target2& t, float2 dx,
+                                               float2 dy, float2 dz, float2 rinv, ff_acc2& s)
+{
+    const float2 mx = make_float2(q1.z, q1.w), my = make_float2(q2.x, q2.y), mz = make_float2(q2.z, q2.w);
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 rinv3 = __fmul2_rn(rinv2, rinv);
+    const float2 r5 = __fmul2_rn(rinv3, __fmul2_rn(rinv2, ff_dup(3.0f)));         // 3 / r^5
+    const float2 a = __ffma2_rn(mz, dz, __ffma2_rn(my, dy, __fmul2_rn(mx, dx)));   // u_j . rho
+    const float2 b = __ffma2_rn(t.uz, dz, __ffma2_rn(t.uy, dy, __fmul2_rn(t.ux, dx)));   // u_k . rho
+    const float2 c = __ffma2_rn(mz, t.uz, __ffma2_rn(my, t.uy, __fmul2_rn(mx, t.ux)));   // u_j . u_k
+    const float2 ca = __fmul2_rn(a, r5);
+    const float2 cb = __fmul2_rn(b, r5);
+    const float2 nr3 = __fmul2_rn(rinv2, make_float2(-rinv.x, -rinv.y));           // -1 / r^3 (negation folds into the operand)
+    s.hx = __ffma2_rn(ca, dx, s.hx); s.hy = __ffma2_rn(ca, dy, s.hy); s.hz = __ffma2_rn(ca, dz, s.hz);
+    s.hx = __ffma2_rn(nr3, mx, s.hx); s.hy = __ffma2_rn(nr3, my, s.hy); s.hz = __ffma2_rn(nr3, mz, s.hz);
+    const float2 w = __fmul2_rn(__fmul2_rn(ca, b), rinv2);                         // 3 (u_j.rho)(u_k.rho) / r^7
+    const float2 cr = __ffma2_rn(ff_dup(-5.0f), w, __fmul2_rn(c, r5));
+    s.fx = __ffma2_rn(cr, dx, s.fx); s.fy = __ffma2_rn(cr, dy, s.fy); s.fz = __ffma2_rn(cr, dz, s.fz);
+    s.fx = __ffma2_rn(cb, mx, s.fx); s.fy = __ffma2_rn(cb, my, s.fy); s.fz = __ffma2_rn(cb, mz, s.fz);
+    s.sk = __fadd2_rn(s.sk, ca);
+}

@@ -14,7 +14,7 @@ __global__ void ff_k_reset(ff_globals* g)
     int t = threadIdx.x;
     if (t < 3) { g->bbox_ord[t] = 0xffffffffu; g->bbox_ord[4 + t] = 0u; }
     if (t < 4) g->counters[t] = 0ull;
-    if (t == 0) g->n_cells = 0;
+    if (t == 0) { g->n_cells = 0; g->max_level = 0; }
 }
 
 __global__ void __launch_bounds__(256) ff_k_bbox(const float* __restrict__ pos, int n, ff_globals* g)
@@ -235,12 +235,5 @@ int ff_launch_sort(ff_ctx* c, const float* pos)
     }
     // four passes: the result is back in buffer 0
     FF_LAUNCH(c, ff_k_gather4, (n + 255) / 256, 256, 0, pos, c->idx[0], n, c->pos_s);
-    return FF_OK;
-}
-
-int ff_launch_gather_mom(ff_ctx* c, const float* mom)
-{
-    int n = (int)c->n;
-    FF_LAUNCH(c, ff_k_gather4, (n + 255) / 256, 256, 0, mom, c->idx[0], n, c->mom_s);
     return FF_OK;
 }
