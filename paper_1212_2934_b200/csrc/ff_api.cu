@@ -34,6 +34,7 @@ static size_t carve(ff_ctx* c, char* base, int64_t N)
     p = take(cap * 4);                            if (c) c->cell_first = (int32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_end = (int32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_level = (int32_t*)p;
+    p = take(cap * 4);                            if (c) c->cell_list = (int32_t*)p;
     p = take(cap * 32);                           if (c) c->cell_child = (int32_t*)p;
     p = take(cap * 16);                           if (c) c->cell_centre = (float4*)p;
     p = take(cap * 16);                           if (c) c->cell_moment = (float4*)p;

@@ -18,6 +18,9 @@
 namespace cg = cooperative_groups;
 
 #define FF_MOM_THREADS 256
+#define FF_BUILD_THREADS 256
+#define FF_BUILD_ITEMS 8
+#define FF_BUILD_TILE (FF_BUILD_THREADS * FF_BUILD_ITEMS)
 
 __device__ __forceinline__ int ff_lprev(const uint32_t* __restrict__ key, int i)
 {
@@ -31,85 +34,6 @@ __device__ __forceinline__ int ff_cells_at(const uint32_t* __restrict__ key, int
     return max(0, min(lk, FF_MAX_LEVEL - 1) - lprev);
 }
 
-// ---- device-wide exclusive scan of ff_cells_at (reduce / scan block sums / write) --
-__global__ void __launch_bounds__(FF_SCAN_THREADS)
-ff_k_cells_reduce(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restrict__ blk)
-{
-    __shared__ uint32_t wsum[FF_SCAN_THREADS / 32];
-    uint32_t s = 0;
-    int base = blockIdx.x * FF_SCAN_TILE;
-#pragma unroll
-    for (int r = 0; r < FF_SCAN_ITEMS; ++r) {
-        int i = base + r * FF_SCAN_THREADS + threadIdx.x;
-        int lp;
-        if (i < n) s += (uint32_t)ff_cells_at(key, i, n, nleaf, lp);
-    }
-    s = __reduce_add_sync(FF_FULL, s);
-    if (ff_lane() == 0) wsum[threadIdx.x >> 5] = s;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t t = 0;
-        for (int k = 0; k < FF_SCAN_THREADS / 32; ++k) t += wsum[k];
-        blk[blockIdx.x] = t;
-    }
-}
-
-// single block: exclusive scan of blk[0..m) in place; total -> g->n_cells
-__global__ void __launch_bounds__(1024) ff_k_scan_blocksums(uint32_t* __restrict__ blk, int m, ff_globals* g)
-{
-    __shared__ uint32_t wsum[32];
-    __shared__ uint32_t carry_s;
-    int lane = ff_lane(), w = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (int base = 0; base < m; base += 1024) {
-        int i = base + threadIdx.x;
-        uint32_t v = i < m ? blk[i] : 0u, x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FF_FULL, x, o); if (lane >= o) x += y; }
-        if (lane == 31) wsum[w] = x;
-        __syncthreads();
-        uint32_t woff = 0, tot = 0;
-        for (int k = 0; k < 32; ++k) { uint32_t s = wsum[k]; if (k < w) woff += s; tot += s; }
-        uint32_t carry = carry_s;
-        if (i < m) blk[i] = carry + woff + x - v;
-        __syncthreads();
-        if (threadIdx.x == 0) carry_s = carry + tot;
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) g->n_cells = (int32_t)carry_s;
-}
-
-// per tile: exclusive scan in slot order (thread t owns FF_SCAN_ITEMS consecutive slots)
-__global__ void __launch_bounds__(FF_SCAN_THREADS)
-ff_k_cells_scan(const uint32_t* __restrict__ key, int n, int nleaf, const uint32_t* __restrict__ blk,
-                int32_t* __restrict__ cell_base)
-{
-    __shared__ uint32_t wsum[FF_SCAN_THREADS / 32];
-    int lane = ff_lane(), w = threadIdx.x >> 5;
-    int first = blockIdx.x * FF_SCAN_TILE + threadIdx.x * FF_SCAN_ITEMS;
-    uint32_t c[FF_SCAN_ITEMS], s = 0;
-#pragma unroll
-    for (int r = 0; r < FF_SCAN_ITEMS; ++r) {
-        int i = first + r, lp;
-        c[r] = i < n ? (uint32_t)ff_cells_at(key, i, n, nleaf, lp) : 0u;
-        s += c[r];
-    }
-    uint32_t x = s;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FF_FULL, x, o); if (lane >= o) x += y; }
-    if (lane == 31) wsum[w] = x;
-    __syncthreads();
-    uint32_t run = blk[blockIdx.x] + x - s;
-    for (int k = 0; k < w; ++k) run += wsum[k];
-#pragma unroll
-    for (int r = 0; r < FF_SCAN_ITEMS; ++r) {
-        int i = first + r;
-        if (i < n) cell_base[i] = (int32_t)run;
-        run += c[r];
-    }
-}
-
 // first slot in [lo, hi) whose key is >= bound (keys sorted ascending)
 __device__ __forceinline__ int ff_lower_bound(const uint32_t* __restrict__ key, int lo, int hi, uint32_t bound)
 {
@@ -120,57 +44,168 @@ __device__ __forceinline__ int ff_lower_bound(const uint32_t* __restrict__ key, 
     return lo;
 }
 
-// ---- a4: one thread per slot writes the internal cells that start there -----------
-__global__ void __launch_bounds__(128)
-ff_k_cells_fill(const uint32_t* __restrict__ key, int n, int nleaf, const int32_t* __restrict__ cell_base,
-                int32_t* __restrict__ cell_first, int32_t* __restrict__ cell_end, int32_t* __restrict__ cell_level,
-                int32_t* __restrict__ cell_child, int32_t* __restrict__ leaf_count, int cell_cap, ff_globals* g)
+// the same, galloping up from lo: ~2 log2(answer - lo) probes, short for the many small cells
+__device__ __forceinline__ int ff_gallop_bound(const uint32_t* __restrict__ key, int lo, int n, uint32_t bound)
 {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    int lprev;
-    int cnt = ff_cells_at(key, i, n, nleaf, lprev);
-    {   // deepest level holding an internal cell (bounds the level loop of ff_k_moments)
-        int deepest = __reduce_max_sync(__activemask(), cnt > 0 ? lprev + cnt : 0);
-        if (ff_lane() == 0 && deepest > 0) atomicMax(&g->max_level, deepest);
+    int pos = lo, step = 1;
+    while (pos < n && __ldg(key + pos) < bound) { lo = pos + 1; pos += step; step <<= 1; }
+    return ff_lower_bound(key, lo, min(pos, n), bound);
+}
+
+// ---- a4: the whole octree build as ONE cooperative launch ---------------------------------
+//   phase 1  every block counts the cells that start in its contiguous range of slots
+//   phase 2  exclusive scan (block prefix + in-tile scan) -> cell_base[slot]; every cell gets
+//            its first slot and level; level histogram
+//   phase 3  eight lanes per cell: lane o finds the end of octant o with a galloping search in
+//            the sorted keys (one search per lane, all of similar length), which gives the cell's
+//            range and its eight child links; the cell's id is appended to its level's list
+//            (ff_k_moments walks the levels deepest first)
+// The paper builds the tree by locked insertion (kernel 2); no locks here, and
+// the result does not depend on scheduling except for the order inside a level list, which no
+// result depends on.
+__global__ void __launch_bounds__(FF_BUILD_THREADS)
+ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restrict__ blk,
+           int32_t* __restrict__ cell_base, int32_t* __restrict__ cell_first, int32_t* __restrict__ cell_end,
+           int32_t* __restrict__ cell_level, int32_t* __restrict__ cell_child, int32_t* __restrict__ leaf_count,
+           int32_t* __restrict__ cell_list, int cell_cap, ff_globals* g)
+{
+    cg::grid_group grid = cg::this_grid();
+    __shared__ uint32_t wsum[FF_BUILD_THREADS / 32];
+    __shared__ uint32_t s_bcast[2];
+    __shared__ int s_hist[FF_MAX_LEVEL], s_cur[FF_MAX_LEVEL];
+    const int lane = ff_lane(), w = threadIdx.x >> 5;
+    const int tiles = (n + FF_BUILD_TILE - 1) / FF_BUILD_TILE;
+    const int tpb = (tiles + gridDim.x - 1) / gridDim.x;
+    const int t0 = min(tiles, (int)blockIdx.x * tpb), t1 = min(tiles, t0 + tpb);
+
+    // ---- phase 1
+    {
+        uint32_t s = 0;
+        for (int t = t0; t < t1; ++t) {
+#pragma unroll
+            for (int r = 0; r < FF_BUILD_ITEMS; ++r) {
+                int i = t * FF_BUILD_TILE + r * FF_BUILD_THREADS + threadIdx.x, lp;
+                if (i < n) s += (uint32_t)ff_cells_at(key, i, n, nleaf, lp);
+            }
+        }
+        s = __reduce_add_sync(FF_FULL, s);
+        if (lane == 0) wsum[w] = s;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            uint32_t t = 0;
+            for (int k = 0; k < FF_BUILD_THREADS / 32; ++k) t += wsum[k];
+            blk[blockIdx.x] = t;
+        }
     }
-    if (cnt == 0) return;
-    int base = cell_base[i];
-    if (base + cnt > cell_cap) { g->error = FF_ERR_CAPACITY; return; }
-    uint32_t k = __ldg(key + i);
-    int end_parent = n;                                    // end of the enclosing cell: search bound
-    for (int q = 0; q < cnt; ++q) {
-        int l = lprev + 1 + q;
-        int id = base + q;
-        int sh = 3 * (FF_MAX_LEVEL - l);                   // bits below the level-l prefix
-        int end;
-        if (l == 0) end = n;
-        else {
-            uint32_t bound = ((k >> sh) + 1u) << sh;       // first key past this cell (no overflow: 30-bit keys)
-            end = ff_lower_bound(key, i + 1, end_parent, bound);
+    grid.sync();
+
+    // ---- phase 2
+    {
+        uint32_t before = 0, total = 0;
+        for (int j = threadIdx.x; j < (int)gridDim.x; j += FF_BUILD_THREADS) {
+            uint32_t v = blk[j];
+            total += v;
+            if (j < (int)blockIdx.x) before += v;
         }
-        end_parent = end;
-        cell_first[id] = i;
-        cell_end[id] = end;
-        cell_level[id] = l;
-        // children: octant boundaries inside [i, end)
-        int csh = sh - 3;
-        uint32_t cpre = (k >> sh) << 3;                    // child prefix without the octant
-        int b = i;
-        for (int o = 0; o < 8; ++o) {
-            int e = (o == 7) ? end : ff_lower_bound(key, b, end, (cpre + (uint32_t)o + 1u) << csh);
-            int cc = e - b;
-            int32_t ent;
-            if (cc == 0) ent = FF_CHILD_EMPTY;
-            else if (cc > nleaf && l + 1 < FF_MAX_LEVEL) {
-                // internal child: starts at slot b on level l+1
-                int lp = ff_lprev(key, b);
-                ent = cell_base[b] + (l + 1 - lp - 1);
-            } else if (cc == 1) ent = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)b);
-            else { ent = (int32_t)(FF_CHILD_LEAF1 | FF_CHILD_MULTI | (uint32_t)b); leaf_count[b] = cc; }
-            cell_child[8 * (size_t)id + o] = ent;
-            b = e;
+        before = __reduce_add_sync(FF_FULL, before);
+        total = __reduce_add_sync(FF_FULL, total);
+        __syncthreads();
+        if (threadIdx.x < 2) s_bcast[threadIdx.x] = 0;
+        if (threadIdx.x < FF_MAX_LEVEL) s_hist[threadIdx.x] = 0;
+        __syncthreads();
+        if (lane == 0) { atomicAdd(&s_bcast[0], before); atomicAdd(&s_bcast[1], total); }
+        __syncthreads();
+        uint32_t carry = s_bcast[0];
+        total = s_bcast[1];
+        const bool fits = total <= (uint32_t)cell_cap;
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            g->n_cells = fits ? (int32_t)total : 0;
+            if (!fits) g->error = FF_ERR_CAPACITY;
         }
+        for (int t = t0; t < t1; ++t) {
+            const int first = t * FF_BUILD_TILE + threadIdx.x * FF_BUILD_ITEMS;
+            uint32_t c[FF_BUILD_ITEMS], s = 0;
+            int lp[FF_BUILD_ITEMS];
+#pragma unroll
+            for (int r = 0; r < FF_BUILD_ITEMS; ++r) {
+                int i = first + r;
+                lp[r] = 0;
+                c[r] = i < n ? (uint32_t)ff_cells_at(key, i, n, nleaf, lp[r]) : 0u;
+                s += c[r];
+            }
+            uint32_t x = s;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FF_FULL, x, o); if (lane >= o) x += y; }
+            __syncthreads();                               // wsum of the previous tile fully read
+            if (lane == 31) wsum[w] = x;
+            __syncthreads();
+            uint32_t run = carry + x - s, tile_total = 0;
+            for (int k = 0; k < FF_BUILD_THREADS / 32; ++k) { uint32_t v = wsum[k]; if (k < w) run += v; tile_total += v; }
+#pragma unroll
+            for (int r = 0; r < FF_BUILD_ITEMS; ++r) {
+                int i = first + r;
+                if (i < n) cell_base[i] = (int32_t)run;
+                if (fits)
+                    for (uint32_t q = 0; q < c[r]; ++q) {
+                        int l = lp[r] + 1 + (int)q;
+                        cell_first[run + q] = i;
+                        cell_level[run + q] = l;
+                        atomicAdd(&s_hist[l], 1);
+                    }
+                run += c[r];
+            }
+            carry += tile_total;
+        }
+        __syncthreads();
+        if (threadIdx.x < FF_MAX_LEVEL && s_hist[threadIdx.x]) atomicAdd(&g->level_count[threadIdx.x], s_hist[threadIdx.x]);
+    }
+    grid.sync();
+
+    // ---- phase 3
+    const int n_cells = g->n_cells;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int run = 0, deepest = 0;
+        for (int l = 0; l < FF_MAX_LEVEL; ++l) {
+            s_cur[l] = run;                                // start of level l in cell_list
+            if (blockIdx.x == 0) g->level_start[l] = run;
+            int cnt = g->level_count[l];
+            if (cnt > 0) deepest = l;
+            run += cnt;
+        }
+        if (blockIdx.x == 0) { g->level_start[FF_MAX_LEVEL] = run; g->max_level = deepest; }
+    }
+    if (threadIdx.x < FF_MAX_LEVEL) s_hist[threadIdx.x] = 0;
+    __syncthreads();
+    const int cpb = (n_cells + gridDim.x - 1) / gridDim.x;
+    const int c0 = min(n_cells, (int)blockIdx.x * cpb), c1 = min(n_cells, c0 + cpb);
+    for (int id = c0 + threadIdx.x; id < c1; id += FF_BUILD_THREADS) atomicAdd(&s_hist[cell_level[id]], 1);
+    __syncthreads();
+    if (threadIdx.x < FF_MAX_LEVEL && s_hist[threadIdx.x])
+        s_cur[threadIdx.x] += atomicAdd(&g->level_cursor[threadIdx.x], s_hist[threadIdx.x]);
+    __syncthreads();
+    const int o = threadIdx.x & 7;
+    const unsigned gmask = 0xffu << (threadIdx.x & 24);
+    for (int id = c0 + (threadIdx.x >> 3); id < c1; id += FF_BUILD_THREADS / 8) {
+        const int first = cell_first[id], l = cell_level[id];
+        const uint32_t k = __ldg(key + first);
+        const int sh = 3 * (FF_MAX_LEVEL - l);             // bits below the level-l prefix
+        const int csh = sh - 3;
+        const uint32_t cpre = (k >> sh) << 3;              // child prefix without the octant
+        // end of octant o = first key >= (cpre + o + 1) << csh; for o = 7 that is the end of the cell
+        // (no overflow: 30-bit keys, the largest bound is 1 << 30)
+        const int e = ff_gallop_bound(key, first, n, (cpre + (uint32_t)o + 1u) << csh);
+        int b = __shfl_up_sync(gmask, e, 1, 8);
+        if (o == 0) b = first;
+        const int cc = e - b;
+        int32_t ent;
+        if (cc == 0) ent = FF_CHILD_EMPTY;
+        else if (cc > nleaf && l + 1 < FF_MAX_LEVEL) ent = cell_base[b] + (l - ff_lprev(key, b));   // internal child: level l+1 at slot b
+        else if (cc == 1) ent = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)b);
+        else { ent = (int32_t)(FF_CHILD_LEAF1 | FF_CHILD_MULTI | (uint32_t)b); leaf_count[b] = cc; }
+        cell_child[8 * (size_t)id + o] = ent;
+        if (o == 7) cell_end[id] = e;
+        if (o == 0) cell_list[atomicAdd(&s_cur[l], 1)] = id;
     }
 }
 
@@ -184,7 +219,7 @@ ff_k_cells_fill(const uint32_t* __restrict__ key, int n, int nleaf, const int32_
 __global__ void __launch_bounds__(FF_MOM_THREADS)
 ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, int n, ff_globals* __restrict__ g,
              const int32_t* __restrict__ cell_first, const int32_t* __restrict__ cell_end,
-             const int32_t* __restrict__ cell_level, const int32_t* __restrict__ cell_child,
+             const int32_t* __restrict__ cell_list, const int32_t* __restrict__ cell_child,
              const int32_t* __restrict__ leaf_count, const float4* __restrict__ pos_s, float4* __restrict__ mom_s,
              double* __restrict__ sum_u, double* __restrict__ sum_p, float4* __restrict__ centre,
              float4* __restrict__ moment)
@@ -196,7 +231,6 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
         mom_s[s] = make_float4(__ldg(mom + j), __ldg(mom + j + 1), __ldg(mom + j + 2), 0.0f);
     }
     if (tid == 0) g->walk_next = 0;                        // the walk's group counter (this is the last launch before it)
-    const int n_cells = g->n_cells;
     const int top = min(g->max_level, FF_MAX_LEVEL - 1);   // deepest level that holds an internal cell
     const float S = g->S;
     // Eight lanes per cell: lane o loads child o (one exposed memory latency per cell instead of eight),
@@ -212,8 +246,9 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
     for (int level = top; level >= 0; --level) {
         const float s = ldexpf(S, -level);
         const float s2 = __fmul_rn(s, s);
-        for (int id = gid; id < n_cells; id += ngroups) {
-            if (cell_level[id] != level) continue;         // uniform over the group's eight lanes
+        const int ls = g->level_start[level], le = g->level_start[level + 1];
+        for (int k = ls + gid; k < le; k += ngroups) {
+            const int id = cell_list[k];
             const int32_t e = cell_child[8 * (size_t)id + o];
             const bool have = e != FF_CHILD_EMPTY;
             if (e >= 0) {
@@ -258,12 +293,20 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
 int ff_launch_build(ff_ctx* c)
 {
     int n = (int)c->n;
-    int tiles = (n + FF_SCAN_TILE - 1) / FF_SCAN_TILE;
-    FF_LAUNCH(c, ff_k_cells_reduce, tiles, FF_SCAN_THREADS, 0, c->key[0], n, c->nleaf, c->scan_blk);
-    FF_LAUNCH(c, ff_k_scan_blocksums, 1, 1024, 0, c->scan_blk, tiles, c->g);
-    FF_LAUNCH(c, ff_k_cells_scan, tiles, FF_SCAN_THREADS, 0, c->key[0], n, c->nleaf, c->scan_blk, c->cell_base);
-    FF_LAUNCH(c, ff_k_cells_fill, (n + 127) / 128, 128, 0, c->key[0], n, c->nleaf, c->cell_base, c->cell_first,
-              c->cell_end, c->cell_level, c->cell_child, c->leaf_count, (int)c->cell_cap, c->g);
+    static int per_sm = 0;
+    if (!per_sm) {
+        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_build, FF_BUILD_THREADS, 0));
+        if (per_sm < 1) return FF_ERR_CUDA;
+    }
+    int tiles = (n + FF_BUILD_TILE - 1) / FF_BUILD_TILE;
+    int blocks = min(tiles, c->num_sms * min(per_sm, 8));
+    int nleaf = c->nleaf, cap = (int)c->cell_cap;
+    void* args[] = { (void*)&c->key[0], (void*)&n, (void*)&nleaf, (void*)&c->scan_blk, (void*)&c->cell_base,
+                     (void*)&c->cell_first, (void*)&c->cell_end, (void*)&c->cell_level, (void*)&c->cell_child,
+                     (void*)&c->leaf_count, (void*)&c->cell_list, (void*)&cap, (void*)&c->g };
+    FF_CUDA(c, cudaLaunchCooperativeKernel((const void*)ff_k_build, dim3(blocks), dim3(FF_BUILD_THREADS), args, 0,
+                                           c->stream));
+    c->launches++;
     return FF_OK;
 }
 
@@ -278,7 +321,7 @@ int ff_launch_moments(ff_ctx* c, const float* mom)
     int blocks = min((n + FF_MOM_THREADS - 1) / FF_MOM_THREADS, c->num_sms * min(per_sm, 8));
     const uint32_t* perm = c->idx[0];
     void* args[] = { (void*)&mom, (void*)&perm, (void*)&n, (void*)&c->g, (void*)&c->cell_first, (void*)&c->cell_end,
-                     (void*)&c->cell_level, (void*)&c->cell_child, (void*)&c->leaf_count, (void*)&c->pos_s,
+                     (void*)&c->cell_list, (void*)&c->cell_child, (void*)&c->leaf_count, (void*)&c->pos_s,
                      (void*)&c->mom_s, (void*)&c->cell_sum_u, (void*)&c->cell_sum_p, (void*)&c->cell_centre,
                      (void*)&c->cell_moment };
     FF_CUDA(c, cudaLaunchCooperativeKernel((const void*)ff_k_moments, dim3(blocks), dim3(FF_MOM_THREADS), args, 0,

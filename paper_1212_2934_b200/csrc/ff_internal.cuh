@@ -50,7 +50,10 @@ struct ff_globals {
     float inv;                // fl(1024 / S)
     int32_t n_cells;          // internal cells of the current tree
     int32_t error;            // sticky device-side error flag (FF_ERR_*)
-    int32_t max_level;        // deepest level holding an internal cell (atomicMax in ff_k_cells_fill)
+    int32_t max_level;        // deepest level holding an internal cell
+    int32_t level_count[FF_MAX_LEVEL];      // internal cells per level (ff_k_build)
+    int32_t level_cursor[FF_MAX_LEVEL];     // fill cursors of the level lists
+    int32_t level_start[FF_MAX_LEVEL + 1];  // cell_list[level_start[l] .. level_start[l+1]) = the cells of level l
     int32_t walk_next;        // next target group of the persistent walk (zeroed by the level-0 moment launch)
     unsigned long long counters[4];   // n_cell, n_particle, n_mac, n_parked (FF_OPT_COUNTERS)
     uint32_t digit_total[FF_RADIX];   // per-pass digit totals (ff_sort.cu)
@@ -82,6 +85,7 @@ struct ff_ctx {
     uint32_t* scan_blk;               // block sums of the scan
     uint32_t* sort_hist;              // [FF_RADIX][n_tiles]
     int32_t *cell_first, *cell_end, *cell_level;
+    int32_t* cell_list;               // [cap] cell ids grouped by level
     int32_t* cell_child;              // [cap][8]
     float4 *cell_centre, *cell_moment;
     double *cell_sum_u, *cell_sum_p;  // [cap][3] fp64 sums in the fixed order

@@ -15,6 +15,7 @@ __global__ void ff_k_reset(ff_globals* g)
     if (t < 3) { g->bbox_ord[t] = 0xffffffffu; g->bbox_ord[4 + t] = 0u; }
     if (t < 4) g->counters[t] = 0ull;
     if (t == 0) { g->n_cells = 0; g->max_level = 0; }
+    if (t < FF_MAX_LEVEL) { g->level_count[t] = 0; g->level_cursor[t] = 0; }
 }
 
 __global__ void __launch_bounds__(256) ff_k_bbox(const float* __restrict__ pos, int n, ff_globals* g)
