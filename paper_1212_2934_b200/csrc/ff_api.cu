@@ -30,7 +30,7 @@ static size_t carve(ff_ctx* c, char* base, int64_t N)
     p = take(n * 4);                              if (c) c->leaf_count = (int32_t*)p;
     p = take(n * 4);                              if (c) c->cell_base = (int32_t*)p;
     p = take((scan_tiles + 1) * 4);               if (c) c->scan_blk = (uint32_t*)p;
-    p = take(sort_tiles * FF_RADIX * 4);          if (c) c->sort_hist = (uint32_t*)p;
+    p = take(sort_tiles * FF_RADIX * 4 * FF_SORT_PASSES); if (c) c->sort_status = (uint32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_first = (int32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_end = (int32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_level = (int32_t*)p;

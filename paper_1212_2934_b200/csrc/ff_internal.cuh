@@ -17,6 +17,7 @@
 #define FF_SORT_TILE (FF_SORT_THREADS * FF_SORT_ROUNDS)    // keys per block
 #define FF_RADIX_BITS 8
 #define FF_RADIX 256
+#define FF_SORT_PASSES 4
 
 // ---- scan geometry (ff_build.cu) --------------------------------------------
 #define FF_SCAN_THREADS 256
@@ -56,7 +57,8 @@ struct ff_globals {
     int32_t level_start[FF_MAX_LEVEL + 1];  // cell_list[level_start[l] .. level_start[l+1]) = the cells of level l
     int32_t walk_next;        // next target group of the persistent walk (zeroed by the level-0 moment launch)
     unsigned long long counters[4];   // n_cell, n_particle, n_mac, n_parked (FF_OPT_COUNTERS)
-    uint32_t digit_total[FF_RADIX];   // per-pass digit totals (ff_sort.cu)
+    int32_t sort_ticket[FF_SORT_PASSES];              // next tile of each sort pass
+    uint32_t digit_hist[FF_SORT_PASSES][FF_RADIX];    // global digit histograms of the four passes (ff_k_keys)
 };
 
 struct ff_ctx {
@@ -83,7 +85,7 @@ struct ff_ctx {
     int32_t* leaf_count;              // [N]
     int32_t* cell_base;               // [N] exclusive scan of cells starting at each slot
     uint32_t* scan_blk;               // block sums of the scan
-    uint32_t* sort_hist;              // [FF_RADIX][n_tiles]
+    uint32_t* sort_status;            // [FF_SORT_PASSES][n_tiles][FF_RADIX] look-back status words
     int32_t *cell_first, *cell_end, *cell_level;
     int32_t* cell_list;               // [cap] cell ids grouped by level
     int32_t* cell_child;              // [cap][8]

@@ -16,6 +16,8 @@ __global__ void ff_k_reset(ff_globals* g)
     if (t < 4) g->counters[t] = 0ull;
     if (t == 0) { g->n_cells = 0; g->max_level = 0; }
     if (t < FF_MAX_LEVEL) { g->level_count[t] = 0; g->level_cursor[t] = 0; }
+    if (t < FF_SORT_PASSES) g->sort_ticket[t] = 0;
+    (&g->digit_hist[0][0])[t] = 0u;                        // launched with FF_SORT_PASSES * FF_RADIX threads
 }
 
 __global__ void __launch_bounds__(256) ff_k_bbox(const float* __restrict__ pos, int n, ff_globals* g)
@@ -71,91 +73,73 @@ __device__ __forceinline__ void ff_root_cube(const ff_globals* g, float lo[3], f
     inv = __fdiv_rn(1024.0f, S);
 }
 
+// Also: the digit histograms of all four sort passes (they do not depend on the order of the keys,
+// so one read of the keys serves every pass) and the reset of the sort's tile-status words.
 __global__ void __launch_bounds__(256) ff_k_keys(const float* __restrict__ pos, int n, ff_globals* g,
-                                                 uint32_t* __restrict__ key)
+                                                 uint32_t* __restrict__ key, uint32_t* __restrict__ status,
+                                                 int n_status)
 {
+    __shared__ uint32_t h[FF_SORT_PASSES][FF_RADIX];
+#pragma unroll
+    for (int p = 0; p < FF_SORT_PASSES; ++p) h[p][threadIdx.x] = 0;
     float lo[3], S, inv;
     ff_root_cube(g, lo, S, inv);
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i == 0) { g->lo[0] = lo[0]; g->lo[1] = lo[1]; g->lo[2] = lo[2]; g->S = S; g->inv = inv; }
-    if (i >= n) return;
-    uint32_t q[3];
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    if (tid == 0) { g->lo[0] = lo[0]; g->lo[1] = lo[1]; g->lo[2] = lo[2]; g->S = S; g->inv = inv; }
+    for (int i = tid; i < n_status; i += nth) status[i] = 0u;
+    __syncthreads();
+    for (int i = tid; i < n; i += nth) {
+        uint32_t q[3];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        float d = __fsub_rn(__ldg(pos + 3 * (size_t)i + a), lo[a]);
-        int v = __float2int_rd(__fmul_rn(d, inv));      // floor, then to int
-        q[a] = (uint32_t)min(1023, max(0, v));
+        for (int a = 0; a < 3; ++a) {
+            float d = __fsub_rn(__ldg(pos + 3 * (size_t)i + a), lo[a]);
+            int v = __float2int_rd(__fmul_rn(d, inv));      // floor, then to int
+            q[a] = (uint32_t)min(1023, max(0, v));
+        }
+        const uint32_t k = (ff_spread10(q[0]) << 2) | (ff_spread10(q[1]) << 1) | ff_spread10(q[2]);
+        key[i] = k;
+#pragma unroll
+        for (int p = 0; p < FF_SORT_PASSES; ++p) atomicAdd(&h[p][(k >> (p * FF_RADIX_BITS)) & (FF_RADIX - 1)], 1u);
     }
-    key[i] = (ff_spread10(q[0]) << 2) | (ff_spread10(q[1]) << 1) | ff_spread10(q[2]);
+    __syncthreads();
+#pragma unroll
+    for (int p = 0; p < FF_SORT_PASSES; ++p)
+        if (h[p][threadIdx.x]) atomicAdd(&g->digit_hist[p][threadIdx.x], h[p][threadIdx.x]);
 }
 
 // ------------------------------------------------------------ a3 radix sort --
-// LSD, 8-bit digits, 4 passes over the 30-bit key.  Per pass: (1) per-tile digit
-// histogram, (2) per-digit exclusive scan over tiles, (3) stable scatter using
-// warp match ranking.  Stability within a tile: a warp owns a contiguous chunk
-// and walks it in rounds of 32; rank = earlier rounds' count + lower lanes.
-__global__ void __launch_bounds__(FF_SORT_THREADS)
-ff_k_radix_hist(const uint32_t* __restrict__ key, int n, int shift, uint32_t mask,
-                uint32_t* __restrict__ hist, int n_tiles)
-{
-    __shared__ uint32_t h[FF_RADIX];
-    h[threadIdx.x] = 0;
-    __syncthreads();
-    int lane = ff_lane(), w = threadIdx.x >> 5;
-    int base = blockIdx.x * FF_SORT_TILE + w * 32 * FF_SORT_ROUNDS;
-#pragma unroll
-    for (int r = 0; r < FF_SORT_ROUNDS; ++r) {
-        int i = base + r * 32 + lane;
-        bool valid = i < n;
-        uint32_t d = valid ? ((__ldg(key + i) >> shift) & mask) : 0xffffffffu;
-        unsigned peers = __match_any_sync(FF_FULL, d);
-        if (valid && lane == __ffs(peers) - 1) atomicAdd(&h[d], (uint32_t)__popc(peers));
-    }
-    __syncthreads();
-    hist[(size_t)threadIdx.x * n_tiles + blockIdx.x] = h[threadIdx.x];
-}
-
-// one block per digit: exclusive scan of hist[d][0..n_tiles) in place, total -> g->digit_total[d]
-__global__ void __launch_bounds__(256) ff_k_radix_scan(uint32_t* __restrict__ hist, int n_tiles, ff_globals* g)
-{
-    __shared__ uint32_t wsum[8];
-    __shared__ uint32_t carry_s;
-    uint32_t* row = hist + (size_t)blockIdx.x * n_tiles;
-    int lane = ff_lane(), w = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (int base = 0; base < n_tiles; base += 256) {
-        int i = base + threadIdx.x;
-        uint32_t v = i < n_tiles ? row[i] : 0u;
-        uint32_t x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FF_FULL, x, o); if (lane >= o) x += y; }
-        if (lane == 31) wsum[w] = x;
-        __syncthreads();
-        uint32_t woff = 0, tot = 0;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) { uint32_t s = wsum[k]; if (k < w) woff += s; tot += s; }
-        uint32_t carry = carry_s;
-        if (i < n_tiles) row[i] = carry + woff + x - v;
-        __syncthreads();
-        if (threadIdx.x == 0) carry_s = carry + tot;
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) g->digit_total[blockIdx.x] = carry_s;
-}
+// LSD, 8-bit digits, four passes over the 30-bit key, each pass ONE kernel that reads and writes
+// every (key, index) pair once ("onesweep"): the global digit histograms come from ff_k_keys, and
+// the offset of a tile inside a digit's output range is found by decoupled look-back over the
+// status words of the earlier tiles (per tile and digit: count | state; a tile publishes its own
+// count at once and its inclusive prefix as soon as it knows it).  Tiles are handed out by an
+// atomic ticket, so every tile a block waits for is already running.  Stable: a warp owns a
+// contiguous chunk and walks it in rounds of 32; rank = earlier tiles + earlier warps + earlier
+// rounds + lower lanes (warp match).
+#ifndef FF_SORT_WINDOW
+#define FF_SORT_WINDOW 8
+#endif
+#define FF_ST_AGG 0x40000000u
+#define FF_ST_PREFIX 0x80000000u
+#define FF_ST_COUNT 0x3fffffffu
 
 __global__ void __launch_bounds__(FF_SORT_THREADS)
-ff_k_radix_scatter(const uint32_t* __restrict__ kin, const uint32_t* __restrict__ vin,
-                   uint32_t* __restrict__ kout, uint32_t* __restrict__ vout, int n, int shift, uint32_t mask,
-                   const uint32_t* __restrict__ hist, int n_tiles, const ff_globals* __restrict__ g)
+ff_k_radix_onesweep(const uint32_t* __restrict__ kin, const uint32_t* __restrict__ vin,
+                    uint32_t* __restrict__ kout, uint32_t* __restrict__ vout, int n, int pass,
+                    uint32_t* status, ff_globals* g)
 {
-    __shared__ uint32_t wh[FF_SORT_THREADS / 32][FF_RADIX];   // per-warp digit counts, then bases
+    __shared__ uint32_t wh[FF_SORT_THREADS / 32][FF_RADIX];   // per-warp digit counts, then offsets
+    __shared__ uint32_t tile_base[FF_RADIX];
+    __shared__ uint32_t skey[FF_SORT_TILE], sval[FF_SORT_TILE];
     __shared__ uint32_t wsum[8];
-    int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    __shared__ int s_tile;
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const int shift = pass * FF_RADIX_BITS;
+    if (t == 0) s_tile = atomicAdd(&g->sort_ticket[pass], 1);
 #pragma unroll
     for (int k = 0; k < FF_SORT_THREADS / 32; ++k) wh[k][t] = 0;
-    // exclusive scan of the digit totals -> first output slot of digit t
-    uint32_t tot = g->digit_total[t], x = tot;
+    // exclusive scan of the global digit histogram -> first output slot of digit t
+    uint32_t tot = g->digit_hist[pass][t], x = tot;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FF_FULL, x, o); if (lane >= o) x += y; }
     if (lane == 31) wsum[w] = x;
@@ -163,17 +147,28 @@ ff_k_radix_scatter(const uint32_t* __restrict__ kin, const uint32_t* __restrict_
     uint32_t dbase = x - tot;
 #pragma unroll
     for (int k = 0; k < 8; ++k) if (k < w) dbase += wsum[k];
+    const int tile = s_tile;
 
     uint32_t key[FF_SORT_ROUNDS], val[FF_SORT_ROUNDS], rank[FF_SORT_ROUNDS];
-    int base = blockIdx.x * FF_SORT_TILE + w * 32 * FF_SORT_ROUNDS;
+    const int base = tile * FF_SORT_TILE + w * 32 * FF_SORT_ROUNDS;
 #pragma unroll
     for (int r = 0; r < FF_SORT_ROUNDS; ++r) {
         int i = base + r * 32 + lane;
         bool valid = i < n;
         key[r] = valid ? __ldg(kin + i) : 0xffffffffu;
         val[r] = valid ? (vin ? __ldg(vin + i) : (uint32_t)i) : 0u;
-        uint32_t d = valid ? ((key[r] >> shift) & mask) : 0xffffffffu;
-        unsigned peers = __match_any_sync(FF_FULL, d);
+    }
+#pragma unroll
+    for (int r = 0; r < FF_SORT_ROUNDS; ++r) {
+        bool valid = base + r * 32 + lane < n;
+        uint32_t d = (key[r] >> shift) & (FF_RADIX - 1);
+        // lanes with the same digit, from eight ballots (much faster than MATCH.ANY with ~28 distinct digits per warp)
+        unsigned peers = __ballot_sync(FF_FULL, valid);
+#pragma unroll
+        for (int b = 0; b < FF_RADIX_BITS; ++b) {
+            unsigned bal = __ballot_sync(FF_FULL, (d >> b) & 1u);
+            peers &= ((d >> b) & 1u) ? bal : ~bal;
+        }
         int leader = __ffs(peers) - 1;
         uint32_t old = 0;
         if (valid && lane == leader) { old = wh[w][d]; wh[w][d] = old + (uint32_t)__popc(peers); }
@@ -182,19 +177,70 @@ ff_k_radix_scatter(const uint32_t* __restrict__ kin, const uint32_t* __restrict_
         __syncwarp();
     }
     __syncthreads();
-    // digit t: global base of this tile, then exclusive prefix over the warps
-    uint32_t run = dbase + hist[(size_t)t * n_tiles + blockIdx.x];
+    // digit t: count of this tile; per-warp counts become offsets inside the tile's run of digit t
+    uint32_t cnt = 0;
 #pragma unroll
-    for (int k = 0; k < FF_SORT_THREADS / 32; ++k) { uint32_t c = wh[k][t]; wh[k][t] = run; run += c; }
+    for (int k = 0; k < FF_SORT_THREADS / 32; ++k) { uint32_t c = wh[k][t]; wh[k][t] = cnt; cnt += c; }
+    // decoupled look-back: digits of this tile that precede ... = sum of the counts of tiles < tile
+    volatile uint32_t* st = status + (size_t)tile * FF_RADIX + t;
+    uint32_t excl = 0;
+    if (tile == 0) {
+        *st = cnt | FF_ST_PREFIX;
+    } else {
+        *st = cnt | FF_ST_AGG;
+        // FF_SORT_WINDOW predecessors per step (independent loads: one memory latency per step, not per tile)
+        int j = tile - 1;
+        for (;;) {
+            uint32_t v[FF_SORT_WINDOW];
+#pragma unroll
+            for (int q = 0; q < FF_SORT_WINDOW; ++q)
+                v[q] = j - q >= 0 ? *(volatile uint32_t*)(status + (size_t)(j - q) * FF_RADIX + t) : FF_ST_PREFIX;
+            bool done = false;
+#pragma unroll
+            for (int q = 0; q < FF_SORT_WINDOW; ++q) {
+                if (done || !(v[q] & (FF_ST_PREFIX | FF_ST_AGG))) break;     // not published yet: re-read from here
+                excl += v[q] & FF_ST_COUNT;
+                --j;
+                done = (v[q] & FF_ST_PREFIX) != 0;
+            }
+            if (done) break;
+        }
+        *st = (excl + cnt) | FF_ST_PREFIX;
+    }
+    // Reorder the tile by digit in shared memory, then write runs: consecutive threads write consecutive
+    // slots of a digit's run (about 8 pairs = one 32-byte sector per run instead of one sector per pair).
+    uint32_t lx = cnt;                                     // exclusive scan of the tile's digit counts
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FF_FULL, lx, o); if (lane >= o) lx += y; }
+    __syncthreads();                                       // wsum of the first scan fully read
+    if (lane == 31) wsum[w] = lx;
+    __syncthreads();
+    uint32_t lstart = lx - cnt;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) if (k < w) lstart += wsum[k];
+    tile_base[t] = dbase + excl - lstart;                  // output slot of staged element i with digit t: tile_base[t] + i
+#pragma unroll
+    for (int k = 0; k < FF_SORT_THREADS / 32; ++k) wh[k][t] += lstart;   // staged position = wh[w][d] + rank
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < FF_SORT_ROUNDS; ++r) {
-        int i = base + r * 32 + lane;
-        if (i < n) {
-            uint32_t d = (key[r] >> shift) & mask;
-            uint32_t dst = wh[w][d] + rank[r];
-            kout[dst] = key[r];
-            vout[dst] = val[r];
+        if (base + r * 32 + lane < n) {
+            uint32_t d = (key[r] >> shift) & (FF_RADIX - 1);
+            uint32_t lp = wh[w][d] + rank[r];
+            skey[lp] = key[r];
+            sval[lp] = val[r];
+        }
+    }
+    __syncthreads();
+    const int tile_n = min(FF_SORT_TILE, n - tile * FF_SORT_TILE);
+#pragma unroll
+    for (int r = 0; r < FF_SORT_ROUNDS; ++r) {
+        int i = r * FF_SORT_THREADS + t;
+        if (i < tile_n) {
+            uint32_t k = skey[i];
+            uint32_t dst = tile_base[(k >> shift) & (FF_RADIX - 1)] + (uint32_t)i;
+            kout[dst] = k;
+            vout[dst] = sval[i];
         }
     }
 }
@@ -212,10 +258,11 @@ __global__ void __launch_bounds__(256) ff_k_gather4(const float* __restrict__ in
 int ff_launch_bbox_keys(ff_ctx* c, const float* pos)
 {
     int n = (int)c->n;
-    FF_LAUNCH(c, ff_k_reset, 1, 32, 0, c->g);
+    int n_tiles = (n + FF_SORT_TILE - 1) / FF_SORT_TILE;
+    FF_LAUNCH(c, ff_k_reset, 1, FF_SORT_PASSES * FF_RADIX, 0, c->g);
     int blocks = min((n + 255) / 256, c->num_sms * 8);
     FF_LAUNCH(c, ff_k_bbox, blocks, 256, 0, pos, n, c->g);
-    FF_LAUNCH(c, ff_k_keys, (n + 255) / 256, 256, 0, pos, n, c->g, c->key[0]);
+    FF_LAUNCH(c, ff_k_keys, blocks, 256, 0, pos, n, c->g, c->key[0], c->sort_status, FF_SORT_PASSES * n_tiles * FF_RADIX);
     return FF_OK;
 }
 
@@ -224,14 +271,10 @@ int ff_launch_sort(ff_ctx* c, const float* pos)
     int n = (int)c->n;
     int n_tiles = (n + FF_SORT_TILE - 1) / FF_SORT_TILE;
     int cur = 0;
-    for (int pass = 0; pass < 4; ++pass) {
-        int shift = pass * FF_RADIX_BITS;
-        uint32_t mask = pass == 3 ? 0x3fu : 0xffu;
-        FF_LAUNCH(c, ff_k_radix_hist, n_tiles, FF_SORT_THREADS, 0, c->key[cur], n, shift, mask, c->sort_hist, n_tiles);
-        FF_LAUNCH(c, ff_k_radix_scan, FF_RADIX, 256, 0, c->sort_hist, n_tiles, c->g);
-        FF_LAUNCH(c, ff_k_radix_scatter, n_tiles, FF_SORT_THREADS, 0, c->key[cur],
-                  pass == 0 ? (const uint32_t*)nullptr : c->idx[cur], c->key[cur ^ 1], c->idx[cur ^ 1], n, shift, mask,
-                  c->sort_hist, n_tiles, c->g);
+    for (int pass = 0; pass < FF_SORT_PASSES; ++pass) {
+        FF_LAUNCH(c, ff_k_radix_onesweep, n_tiles, FF_SORT_THREADS, 0, c->key[cur],
+                  pass == 0 ? (const uint32_t*)nullptr : c->idx[cur], c->key[cur ^ 1], c->idx[cur ^ 1], n, pass,
+                  c->sort_status + (size_t)pass * n_tiles * FF_RADIX, c->g);
         cur ^= 1;
     }
     // four passes: the result is back in buffer 0
