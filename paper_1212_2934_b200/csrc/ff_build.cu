@@ -18,6 +18,7 @@
 namespace cg = cooperative_groups;
 
 #define FF_MOM_THREADS 256
+#define FF_MOM_SOLO 3                 // levels 0..3 of the moment pass run in one block
 #define FF_BUILD_THREADS 256
 #define FF_BUILD_ITEMS 8
 #define FF_BUILD_TILE (FF_BUILD_THREADS * FF_BUILD_ITEMS)
@@ -244,10 +245,15 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
     const int gid = tid >> 3, ngroups = nth >> 3;
     grid.sync();
     for (int level = top; level >= 0; --level) {
+        // the few cells of levels 0..FF_MOM_SOLO (at most 585) are left to block 0 alone: block-wide
+        // barriers instead of four more grid-wide ones
+        const bool solo = level <= FF_MOM_SOLO;
+        if (solo && blockIdx.x != 0) break;
         const float s = ldexpf(S, -level);
         const float s2 = __fmul_rn(s, s);
         const int ls = g->level_start[level], le = g->level_start[level + 1];
-        for (int k = ls + gid; k < le; k += ngroups) {
+        const int kstep = solo ? FF_MOM_THREADS / 8 : ngroups;
+        for (int k = ls + (solo ? (int)(threadIdx.x >> 3) : gid); k < le; k += kstep) {
             const int id = cell_list[k];
             const int32_t e = cell_child[8 * (size_t)id + o];
             const bool have = e != FF_CHILD_EMPTY;
@@ -286,7 +292,8 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
             else mo[3] = (float)cnt;
             __syncwarp(gmask);                             // smem slots are reused by the group's next cell
         }
-        if (level > 0) grid.sync();
+        if (level > FF_MOM_SOLO) grid.sync();
+        else if (level > 0) __syncthreads();
     }
 }
 
