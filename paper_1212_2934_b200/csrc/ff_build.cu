@@ -18,7 +18,7 @@
 namespace cg = cooperative_groups;
 
 #define FF_MOM_THREADS 256
-#define FF_MOM_SOLO 3                 // levels 0..3 of the moment pass run in one block
+#define FF_MOM_SOLO 1                 // levels 0..1 of the moment pass run in one block
 #define FF_BUILD_THREADS 256
 #define FF_BUILD_ITEMS 8
 #define FF_BUILD_TILE (FF_BUILD_THREADS * FF_BUILD_ITEMS)
@@ -245,8 +245,8 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
     const int gid = tid >> 3, ngroups = nth >> 3;
     grid.sync();
     for (int level = top; level >= 0; --level) {
-        // the few cells of levels 0..FF_MOM_SOLO (at most 585) are left to block 0 alone: block-wide
-        // barriers instead of four more grid-wide ones
+        // the nine cells of levels 0..FF_MOM_SOLO are left to block 0 alone: block-wide barriers
+        // instead of two more grid-wide ones (more levels than that cost more in one block than the barriers)
         const bool solo = level <= FF_MOM_SOLO;
         if (solo && blockIdx.x != 0) break;
         const float s = ldexpf(S, -level);

@@ -51,14 +51,13 @@ __device__ __forceinline__ void ff_pair2_accum(const float4& q1, const float4& q
 {
     const float2 mx = make_float2(q1.z, q1.w), my = make_float2(q2.x, q2.y), mz = make_float2(q2.z, q2.w);
     const float2 rinv2 = __fmul2_rn(rinv, rinv);
-    const float2 rinv3 = __fmul2_rn(rinv2, rinv);
-    const float2 r5 = __fmul2_rn(rinv3, __fmul2_rn(rinv2, ff_dup(3.0f)));         // 3 / r^5
+    const float2 nr3 = __fmul2_rn(rinv2, make_float2(-rinv.x, -rinv.y));           // -1 / r^3 (negation folds into the operand)
+    const float2 r5 = __fmul2_rn(nr3, __fmul2_rn(rinv2, ff_dup(-3.0f)));           // 3 / r^5 = (-1/r^3)(-3/r^2)
     const float2 a = __ffma2_rn(mz, dz, __ffma2_rn(my, dy, __fmul2_rn(mx, dx)));   // u_j . rho
     const float2 b = __ffma2_rn(t.uz, dz, __ffma2_rn(t.uy, dy, __fmul2_rn(t.ux, dx)));   // u_k . rho
     const float2 c = __ffma2_rn(mz, t.uz, __ffma2_rn(my, t.uy, __fmul2_rn(mx, t.ux)));   // u_j . u_k
     const float2 ca = __fmul2_rn(a, r5);
     const float2 cb = __fmul2_rn(b, r5);
-    const float2 nr3 = __fmul2_rn(rinv2, make_float2(-rinv.x, -rinv.y));           // -1 / r^3 (negation folds into the operand)
     s.hx = __ffma2_rn(ca, dx, s.hx); s.hy = __ffma2_rn(ca, dy, s.hy); s.hz = __ffma2_rn(ca, dz, s.hz);
     s.hx = __ffma2_rn(nr3, mx, s.hx); s.hy = __ffma2_rn(nr3, my, s.hy); s.hz = __ffma2_rn(nr3, mz, s.hz);
     const float2 w = __fmul2_rn(__fmul2_rn(ca, b), rinv2);                         // 3 (u_j.rho)(u_k.rho) / r^7
