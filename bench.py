@@ -37,7 +37,7 @@ FLOP_PER_INTERACTION = 60.0      # 21 FFMA x2 + 17 FADD/FMUL + 1 MUFU
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one ff_k_walk launch at config 3, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists)
-WALK_DRAM_TRAFFIC_BYTES = None
+WALK_DRAM_TRAFFIC_BYTES = 107017728   # 84.70 MB read + 22.31 MB written (profiles/r1_walk_full.md)
 
 
 def _peaks():
@@ -280,10 +280,13 @@ def run_ours(args):
         "interactions_per_launch": interactions, "flop_per_interaction": FLOP_PER_INTERACTION,
         "kernel_ms": walk_ms, "kernel_share_of_step": walk_ms / ms_per_step,
         "interactions_per_s": interactions / (walk_ms * 1e-3),
+        "note": "21 of the 38 FP32 instructions per interaction are FMAs, so a saturated FP32 pipe reads 0.78; packed "
+                "FFMA2 with three register-pair operands issues every 3 cycles (profiles/r1_walk_full.md), which caps "
+                "this instruction mix near 0.60",
     }
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     # algorithmic bytes per particle of the HBM-bound phases (DESIGN.md / SURVEY.md 8(d))
-    alg_bytes = {"bbox_keys": 12 + 12 + 4, "sort": 4 * (4 + 16) + 4 + 12 + 16, "build": 26, "moments": 12 + 16 + 122}
+    alg_bytes = {"bbox_keys": 12 + 12 + 4, "sort": 4 * 16 + 4 + 12 + 16, "build": 26, "moments": 12 + 16 + 122}
     hbm_phases = {k: {"ms": phases[k], "achieved_gbs": alg_bytes[k] * N / (phases[k] * 1e-3) / 1e9,
                       "frac_of_hbm_peak": alg_bytes[k] * N / (phases[k] * 1e-3) / 1e9 / hbm}
                   for k in alg_bytes if phases[k] > 0}
