@@ -148,10 +148,11 @@ int ff_eval_direct_host(ff_ctx* ctx, const float* pos_host, const float* mom_hos
  * Q12): rebuilds the tree from pos, evaluates h and f^dip with Barnes-Hut,
  * adds the external field (Eq. 10) and the Lennard-Jones force (Eq. 13,
  * PAPER.md:74, pairs within lj_cutoff), then updates in place
- *   vel    += dtau (f^dip + f^sr - gamma_d vel + noise_d xi)
  *   pos    += dtau vel
- *   angvel += dtau 5/2 (u x h - gamma_r angvel + noise_r xi)
+ *   vel    += dtau (f^dip + f^sr - gamma_d vel) + noise_d sqrt(dtau) xi_d
+ *   angvel += dtau 5/2 (u x h - gamma_r angvel) + noise_r sqrt(dtau) xi_r
  *   mom     = normalise(mom + dtau angvel x mom)
+ * (explicit: every right-hand side uses the values at the start of the step)
  * All arrays device [n][3] fp32.  noise_* = 0 gives the deterministic step
  * used by the parity tests; otherwise xi are unit Gaussians from a
  * counter-based generator keyed by (seed, step_index, particle, component).

@@ -1,0 +1,168 @@
+"""GPU parity of ff_step against oracle/md_step.py + the Barnes-Hut oracle.
+
+One step from a given state is deterministic (noise amplitudes 0): the GPU's new state is compared with the
+oracle's step from the SAME state, with h^dip, f^dip from the oracle's Barnes-Hut at the same theta and group
+width and f^sr from the plain pair sum of Eq. 13.  For a multi-step run the oracle is re-evaluated on the
+GPU's own states (trajectories of a chaotic many-body system are not compared), SURVEY.md 8(d).
+"""
+import numpy as np
+import pytest
+
+import ffgen
+import oracle
+from oracle.md_step import lj_force, md_step
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ff():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1212_2934_b200 as ff
+    ff.lib()
+    return ff
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def _params(ff, **kw):
+    p = ff.ff_step_params()
+    p.dtau = kw.get("dtau", 1e-3)
+    p.gamma_d = kw.get("gamma_d", 0.0)
+    p.gamma_r = kw.get("gamma_r", 0.0)
+    for a in range(3):
+        p.h_ext[a] = kw.get("h_ext", (0.0, 0.0, 0.0))[a]
+    p.lj_epsilon = kw.get("eps", 0.0)
+    p.lj_sigma = kw.get("sigma", 1.0)
+    p.lj_cutoff = kw.get("cutoff", 2.5)
+    p.noise_d = kw.get("noise_d", 0.0)
+    p.noise_r = kw.get("noise_r", 0.0)
+    p.seed = kw.get("seed", 0)
+    return p
+
+
+def _oracle_step(x, v, u, w, theta, kw):
+    """fp64 step from the fp32 state (x, v, u, w) the GPU started from."""
+    H, F, _, _, Q = oracle.barnes_hut(x, u, theta, 32, scale=True)
+    fsr = lj_force(x, kw["eps"], kw["sigma"], kw["cutoff"]) if kw.get("eps", 0.0) != 0.0 else None
+    out = md_step(x, v, u, w, H, F, kw.get("dtau", 1e-3), kw.get("gamma_d", 0.0), kw.get("gamma_r", 0.0),
+                  kw.get("h_ext", (0.0, 0.0, 0.0)), fsr)
+    return out, (H, F, Q, fsr)
+
+
+def _check_step(before, after, ref, aux, kw):
+    """Compare through the increments, which is where the arithmetic of the step sits."""
+    x0, v0, u0, w0 = [a.astype(np.float64) for a in before]
+    x1, v1, u1, w1 = [a.astype(np.float64) for a in after]
+    xr, vr, ur, wr = ref
+    H, F, Q, fsr = aux
+    dt = kw.get("dtau", 1e-3)
+    ulp = 2.0 ** -24
+    # positions: x + dtau v, one fp32 rounding of the result and of the product
+    assert np.abs(x1 - xr).max() <= 4 * ulp * max(1.0, np.abs(xr).max())
+    # velocity increment / dtau = total force - drag: relative to the scale of the force terms
+    acc_gpu, acc_ref = (v1 - v0) / dt, (vr - v0) / dt
+    scale = np.maximum(np.linalg.norm(acc_ref, axis=1), Q[:, 1] / 8.0)
+    if fsr is not None:
+        scale = np.maximum(scale, np.linalg.norm(fsr, axis=1) / 8.0)
+    scale = np.maximum(scale, np.linalg.norm(v0, axis=1) * ulp / dt * 4)       # fp32 rounding of v itself
+    err = np.linalg.norm(acc_gpu - acc_ref, axis=1) / scale
+    assert err.max() <= 2e-4, err.max()
+    # angular-velocity increment / dtau = 5/2 (u x h - Gamma_r omega)
+    t_gpu, t_ref = (w1 - w0) / dt, (wr - w0) / dt
+    tscale = np.maximum(np.linalg.norm(t_ref, axis=1), 2.5 * Q[:, 0] / 8.0)
+    tscale = np.maximum(tscale, np.linalg.norm(w0, axis=1) * ulp / dt * 4)
+    terr = np.linalg.norm(t_gpu - t_ref, axis=1) / tscale
+    assert terr.max() <= 2e-4, terr.max()
+    # moments: unit length, and the same direction as the oracle's
+    assert np.abs(np.linalg.norm(u1, axis=1) - 1.0).max() <= 4 * ulp
+    assert np.abs(u1 - ur).max() <= 8 * ulp
+
+
+KW = dict(dtau=1e-3, gamma_d=0.7, gamma_r=1.3, h_ext=(0.0, 0.1, 0.4), eps=0.5, sigma=1.0, cutoff=2.5)
+
+
+def _state(cfg_id, N, seed):
+    c = ffgen.config(cfg_id, N=N, seed=seed)
+    rng = np.random.default_rng(seed + 100)
+    v = (0.05 * rng.standard_normal((N, 3))).astype(np.float32)
+    w = (0.2 * rng.standard_normal((N, 3))).astype(np.float32)
+    return c["pos"], v, c["mom"], w
+
+
+@pytest.mark.parametrize("cfg_id,N", [(1, 4096), (1, 1531), (2, 6000)])
+def test_one_step_matches_oracle(ff, cfg_id, N):
+    x, v, u, w = _state(cfg_id, N, 0)
+    ctx = ff.FFContext(N, 0.5)
+    dx, dv, du, dw = _dev(x), _dev(v), _dev(u), _dev(w)
+    ctx.step(dx, dv, du, dw, _params(ff, **KW), 0)
+    after = [t.cpu().numpy() for t in (dx, dv, du, dw)]
+    ref, aux = _oracle_step(x, v, u, w, 0.5, KW)
+    _check_step((x, v, u, w), after, ref, aux, KW)
+    # the short-range force is not trivially zero in this test
+    assert np.linalg.norm(aux[3], axis=1).max() > 0.1
+
+
+def test_step_without_short_range_force_and_drag(ff):
+    kw = dict(dtau=2e-3)
+    x, v, u, w = _state(1, 2048, 3)
+    ctx = ff.FFContext(2048, 0.4)
+    dx, dv, du, dw = _dev(x), _dev(v), _dev(u), _dev(w)
+    ctx.step(dx, dv, du, dw, _params(ff, **kw), 0)
+    after = [t.cpu().numpy() for t in (dx, dv, du, dw)]
+    ref, aux = _oracle_step(x, v, u, w, 0.4, kw)
+    _check_step((x, v, u, w), after, ref, aux, kw)
+
+
+def test_twenty_steps_checked_on_the_gpu_states(ff):
+    N = 4096
+    x, v, u, w = _state(1, N, 1)
+    ctx = ff.FFContext(N, 0.5)
+    dx, dv, du, dw = _dev(x), _dev(v), _dev(u), _dev(w)
+    p = _params(ff, **KW)
+    for s in range(20):
+        before = [t.cpu().numpy().copy() for t in (dx, dv, du, dw)]
+        ctx.step(dx, dv, du, dw, p, s)
+        if s in (0, 10, 19):
+            after = [t.cpu().numpy() for t in (dx, dv, du, dw)]
+            ref, aux = _oracle_step(*before, 0.5, KW)
+            _check_step(before, after, ref, aux, KW)
+    # hard spheres at contact with sigma = 1 stay apart over 20 short steps
+    xs = dx.cpu().numpy().astype(np.float64)
+    assert np.isfinite(xs).all()
+
+
+def test_thermal_noise_statistics_and_reproducibility(ff):
+    """xi are unit Gaussians keyed by (seed, step, particle, component): mean 0, variance 1, independent
+    of the launch; the kick is amplitude * sqrt(dtau) * xi (reading Q15)."""
+    import torch
+    N = 1 << 16
+    c = ffgen.config(1, N=4096)
+    x = np.tile(c["pos"], (16, 1)) + np.repeat(np.arange(16), 4096)[:, None].astype(np.float32) * np.float32(100.0)
+    u = np.tile(c["mom"], (16, 1))
+    z = np.zeros((N, 3), np.float32)
+    p = _params(ff, dtau=1e-2, noise_d=0.5, noise_r=0.25, seed=7)
+    q = _params(ff, dtau=1e-2)
+    ctx = ff.FFContext(N, 0.5)
+    outs = []
+    for prm in (p, p, q):
+        dx, dv, du, dw = _dev(x), _dev(z), _dev(u), _dev(z)
+        ctx.step(dx, dv, du, dw, prm, 5)
+        outs.append((dv.cpu().numpy().astype(np.float64), dw.cpu().numpy().astype(np.float64)))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])   # counter-based
+    xi_d = (outs[0][0] - outs[2][0]) / (0.5 * 0.1)
+    xi_r = (outs[0][1] - outs[2][1]) / (0.25 * 0.1)
+    for xi in (xi_d, xi_r):
+        assert abs(xi.mean()) <= 0.01 and abs(xi.var() - 1.0) <= 0.02
+        assert abs(np.mean(xi ** 4) - 3.0) <= 0.15                                   # Gaussian kurtosis
+        cc = np.corrcoef(xi.T)
+        assert np.abs(cc - np.eye(3)).max() <= 0.02
+    assert abs(np.corrcoef(xi_d[:, 0], xi_r[:, 0])[0, 1]) <= 0.02
+    # another step index gives other numbers
+    dx, dv, du, dw = _dev(x), _dev(z), _dev(u), _dev(z)
+    ctx.step(dx, dv, du, dw, p, 6)
+    assert not np.array_equal(dv.cpu().numpy(), outs[0][0].astype(np.float32))
