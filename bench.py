@@ -313,6 +313,35 @@ def run_ours(args):
         ctx.set_option(ff.FF_OPT_THETA, theta)
         extras["bh_vs_allpairs_error"] = {"reference": "GPU direct kernel (ff_eval_direct)", "by_theta": errs}
 
+        # config 3 as BASELINE.json states it: 100 MD steps (ff_step: tree rebuilt, H and F by Barnes-Hut,
+        # Lennard-Jones force, Euler-Maruyama update, dtau = 0.001 as in PAPER.md:200), per-phase timing
+        prm = ff.ff_step_params()
+        prm.dtau, prm.gamma_d, prm.gamma_r = 1e-3, 1.0, 1.0
+        prm.h_ext[0], prm.h_ext[1], prm.h_ext[2] = 0.0, 0.0, 0.5
+        prm.lj_epsilon, prm.lj_sigma, prm.lj_cutoff = 1.0, 1.0, 2.5
+        prm.noise_d, prm.noise_r, prm.seed = 0.05, 0.05, 1
+        x, u = pos.clone(), mom.clone()
+        v, w = torch.zeros_like(pos), torch.zeros_like(pos)
+        for s in range(3):
+            ctx.step(x, v, u, w, prm, s)
+        torch.cuda.synchronize()
+        ctx.timings()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        md_steps = 100
+        e0.record()
+        for s in range(md_steps):
+            ctx.step(x, v, u, w, prm, 3 + s)
+        e1.record()
+        torch.cuda.synchronize()
+        md_ms = e0.elapsed_time(e1) / md_steps
+        last = ctx.timings()
+        extras["md_100_steps"] = {
+            "ms_per_step": md_ms, "particle_steps_per_s": N / (md_ms * 1e-3), "steps": md_steps,
+            "phases_ms_last_step": last, "finite": bool(torch.isfinite(x).all() and torch.isfinite(u).all()),
+            "params": {"dtau": 1e-3, "gamma_d": 1.0, "gamma_r": 1.0, "h_ext": [0, 0, 0.5], "lj": [1.0, 1.0, 2.5],
+                       "noise": [0.05, 0.05]},
+            "note": "L2 not flushed between these steps (back-to-back MD steps, as in a simulation)"}
+
     # ---- the oracle timed beside it on this box's host cores (bounded sample)
     import oracle
     cores = oracle.max_threads()

@@ -63,29 +63,45 @@ ff_k_lj(const uint32_t* __restrict__ key, const float4* __restrict__ pos_s, cons
     float4 p = pos_s[s];
     uint32_t c = __ldg(key + s) >> (3 * (FF_MAX_LEVEL - lev));
     int qx = (int)ff_compact10(c >> 2), qy = (int)ff_compact10(c >> 1), qz = (int)ff_compact10(c);
-    int side = 1 << lev;
+    const int side = 1 << lev;
     float fx = 0.f, fy = 0.f, fz = 0.f;
-    float rc2 = rc * rc, s2 = sigma * sigma;
-    for (int dx = -1; dx <= 1; ++dx)
-        for (int dy = -1; dy <= 1; ++dy)
-            for (int dz = -1; dz <= 1; ++dz) {
-                int x = qx + dx, y = qy + dy, z = qz + dz;
-                if (x < 0 || y < 0 || z < 0 || x >= side || y >= side || z >= side) continue;
-                uint32_t cc = (ff_spread10s((uint32_t)x) << 2) | (ff_spread10s((uint32_t)y) << 1) | ff_spread10s((uint32_t)z);
-                int b = __ldg(start + cc), e = __ldg(end + cc);
-                for (int j = b; j < e; ++j) {
-                    if (j == s) continue;
-                    float4 q = __ldg(pos_s + j);
-                    float rx = p.x - q.x, ry = p.y - q.y, rz = p.z - q.z;
-                    float r2 = fmaf(rz, rz, fmaf(ry, ry, rx * rx));
-                    if (r2 < rc2) {
-                        float ir2 = 1.0f / r2;
-                        float sr2 = s2 * ir2, sr6 = sr2 * sr2 * sr2;
-                        float w = 24.0f * eps * ir2 * (sr6 * sr6 - sr6);
-                        fx = fmaf(w, rx, fx); fy = fmaf(w, ry, fy); fz = fmaf(w, rz, fz);
-                    }
+    const float rc2 = rc * rc, s2 = sigma * sigma, e24 = 24.0f * eps;
+    // Morton codes of the three neighbouring coordinates per axis (0xffffffff = outside the root cube)
+    uint32_t mx[3], my[3], mz[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        int x = qx + d - 1, y = qy + d - 1, z = qz + d - 1;
+        mx[d] = (x < 0 || x >= side) ? 0xffffffffu : ff_spread10s((uint32_t)x) << 2;
+        my[d] = (y < 0 || y >= side) ? 0xffffffffu : ff_spread10s((uint32_t)y) << 1;
+        mz[d] = (z < 0 || z >= side) ? 0xffffffffu : ff_spread10s((uint32_t)z);
+    }
+    // nine (x, y) columns; the table entries of a column's three cells are fetched together, so that a
+    // thread exposes 9 table latencies instead of 27
+#pragma unroll
+    for (int xy = 0; xy < 9; ++xy) {
+        const uint32_t cxy = mx[xy / 3] | my[xy % 3];
+        if (mx[xy / 3] == 0xffffffffu || my[xy % 3] == 0xffffffffu) continue;
+        int b[3], e[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const bool in = mz[d] != 0xffffffffu;
+            b[d] = in ? __ldg(start + (cxy | mz[d])) : 0;
+            e[d] = in ? __ldg(end + (cxy | mz[d])) : 0;
+        }
+#pragma unroll
+        for (int d = 0; d < 3; ++d)
+            for (int j = b[d]; j < e[d]; ++j) {
+                const float4 q = __ldg(pos_s + j);
+                const float rx = p.x - q.x, ry = p.y - q.y, rz = p.z - q.z;
+                const float r2 = fmaf(rz, rz, fmaf(ry, ry, rx * rx));
+                if (r2 < rc2 && j != s) {
+                    const float ir2 = 1.0f / r2;
+                    const float sr2 = s2 * ir2, sr6 = sr2 * sr2 * sr2;
+                    const float w = e24 * ir2 * (sr6 * sr6 - sr6);
+                    fx = fmaf(w, rx, fx); fy = fmaf(w, ry, fy); fz = fmaf(w, rz, fz);
                 }
             }
+    }
     size_t o = (size_t)__ldg(perm + s) * 3;
     fsr[o] = fx; fsr[o + 1] = fy; fsr[o + 2] = fz;
 }
