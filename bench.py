@@ -104,6 +104,29 @@ def _workload(n, seed, cfg=3):
     return c
 
 
+# ---- rank plumbing (one process per GPU; tests/test_multirank.py drives these with gloo on the CPU) ----
+def rank_env():
+    """(world, rank, local_rank) from the torchrun environment; (1, 0, 0) for a plain launch."""
+    return (int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0")),
+            int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def max_over_ranks(ms, world, device):
+    """A time measured on each rank's device -> the slowest rank's time (the job finishes with its last rank)."""
+    import torch
+    t = torch.tensor([float(ms)], device=device, dtype=torch.float64)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_rate(world, units_per_rank, ms):
+    """Whole-job throughput: every rank processed `units_per_rank` units (weak scaling, independent replicas,
+    no data-path collective) in `ms`, the max over ranks."""
+    return world * units_per_rank / (ms * 1e-3)
+
+
 def _describe(c):
     kind = {1: "hard-sphere dipoles (d=1), phi=0.05, isotropic unit moments",
             2: "hard-sphere dipoles (d=1), phi=0.1, von Mises-Fisher moments about +z (kappa=5)",
@@ -172,9 +195,7 @@ def run_ours(args):
 
     import paper_1212_2934_b200 as ff
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local = rank_env()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
     torch.cuda.set_device(local)
@@ -233,14 +254,10 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = float(sum(step_ms))
-    tt = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    total_ms = float(tt.item())
+    total_ms = max_over_ranks(sum(step_ms), world, dev)
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     ms_per_step = total_ms / args.steps
-    value = world * N / (ms_per_step * 1e-3)
+    value = job_rate(world, N, ms_per_step)
     phases = {k: v / args.steps for k, v in phases.items()}
 
     # ---- end to end through the C ABI with host buffers (H2D + step + D2H inside the timed region)
@@ -261,10 +278,7 @@ def run_ours(args):
         e1.record()
         e1.synchronize()
         e2e_ms += e0.elapsed_time(e1)
-    te = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * N / (float(te.item()) / e2e_steps * 1e-3)
+    e2e_value = job_rate(world, N, max_over_ranks(e2e_ms, world, dev) / e2e_steps)
     checksum = float(H_h.double().abs().sum() + F_h.double().abs().sum())
 
     if rank != 0:
