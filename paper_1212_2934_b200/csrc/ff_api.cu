@@ -73,6 +73,8 @@ extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, 
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
     for (int ph = 0; e == cudaSuccess && ph < FF_N_PHASES; ++ph)
         for (int k = 0; e == cudaSuccess && k < 2; ++k) e = cudaEventCreate(&c->ev[ph][k]);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->copy_done, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMemset(c->g, 0, sizeof(ff_globals));
     if (e != cudaSuccess) { delete c; return FF_ERR_CUDA; }
     *out = c;
@@ -85,6 +87,8 @@ extern "C" int ff_destroy(ff_ctx* c)
     cudaStreamSynchronize(c->stream);
     for (int ph = 0; ph < FF_N_PHASES; ++ph)
         for (int k = 0; k < 2; ++k) if (c->ev[ph][k]) cudaEventDestroy(c->ev[ph][k]);
+    if (c->copy_done) cudaEventDestroy(c->copy_done);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
     return FF_OK;
 }
@@ -165,12 +169,17 @@ static int host_roundtrip(ff_ctx* c, const float* pos_h, const float* mom_h, int
     if (!c || !pos_h || !mom_h || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
     size_t bytes = (size_t)n * 12;
     FF_CUDA(c, cudaMemcpyAsync(c->stage_pos, pos_h, bytes, cudaMemcpyHostToDevice, c->stream));
-    FF_CUDA(c, cudaMemcpyAsync(c->stage_mom, mom_h, bytes, cudaMemcpyHostToDevice, c->stream));
     int rc;
     if (bh) {
+        // the moments are not needed before the cell sums: their copy runs on a second stream under the
+        // tree build (the previous call ended with a stream synchronise, so stage_mom is free)
+        FF_CUDA(c, cudaMemcpyAsync(c->stage_mom, mom_h, bytes, cudaMemcpyHostToDevice, c->copy_stream));
+        FF_CUDA(c, cudaEventRecord(c->copy_done, c->copy_stream));
         if ((rc = ff_build_tree(c, c->stage_pos, n)) != FF_OK) return rc;
+        FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->copy_done, 0));
         if ((rc = ff_eval_bh(c, c->stage_pos, c->stage_mom, H_h ? c->stage_H : nullptr, F_h ? c->stage_F : nullptr)) != FF_OK) return rc;
     } else {
+        FF_CUDA(c, cudaMemcpyAsync(c->stage_mom, mom_h, bytes, cudaMemcpyHostToDevice, c->stream));
         if ((rc = ff_eval_direct(c, c->stage_pos, c->stage_mom, n, H_h ? c->stage_H : nullptr, F_h ? c->stage_F : nullptr)) != FF_OK) return rc;
     }
     if (H_h) FF_CUDA(c, cudaMemcpyAsync(H_h, c->stage_H, bytes, cudaMemcpyDeviceToHost, c->stream));

@@ -29,7 +29,7 @@
 #define FF_WALK_WARPS 4            // warps (= target groups) per block
 #endif
 #ifndef FF_WALK_MINB
-#define FF_WALK_MINB 1             // min resident blocks per SM asked of ptxas (register cap)
+#define FF_WALK_MINB 5             // min resident blocks per SM asked of ptxas (caps registers at 96; 5 x 4 warps per SM)
 #endif
 #define FF_WALK_STACK 1024         // traversal stack entries per warp
 #define FF_WALK_PEND 64            // pending interaction ring per warp (two batches of 32)
@@ -74,6 +74,8 @@ struct ff_ctx {
     int device;
     int num_sms;
     cudaStream_t stream;
+    cudaStream_t copy_stream;         // second stream of the *_host calls (moment upload under the tree build)
+    cudaEvent_t copy_done;
     uint64_t launches;
     char last_error[256];
 
