@@ -8,6 +8,12 @@ What is computed, in the paper's notation (all citations are lines of /root/refe
 * lj_force      Eq. 13: f_k^sr = 24 eps sum_{j != k} rho_kj / rho_kj^2 [ (sigma/rho_kj)^12 - (sigma/rho_kj)^6 ],
                 taken literally (no factor 2 on the r^-12 term: the force vanishes at rho = sigma, PAPER.md:52;
                 DESIGN.md reading Q14), restricted to pairs with rho_kj < cutoff (reading Q16).
+* wall_force    PAPER.md:52: "The interaction between a particle and container walls is also modeled with a
+                Lennard-Jones potential of the same type" (containers: PAPER.md:204, a cube and a 2.1 R high
+                monolayer box).  Reading Q20: each of the six planes of an axis-aligned box acts on a
+                particle inside it with the pair term of Eq. 13 evaluated at the distance vector from the plane to
+                the particle centre, f = 24 eps_w n / d [ (sigma_w/d)^12 - (sigma_w/d)^6 ], n = inward normal,
+                for d < cutoff; sigma_w is the centre-to-wall distance at which the force vanishes.
 * md_step       one Euler-Maruyama step of size dtau of Eq. 9 and of the rotational
                 equations in the vector form of DESIGN.md reading Q12 (Eq. 7-8, attach the torque
                 components to the wrong angles; 2/5 = I/(M R^2)):
@@ -44,6 +50,20 @@ def lj_force(pos, eps: float, sigma: float, cutoff: float, chunk: int = 512):
         sr6 = (sigma * sigma / r2) ** 3
         w = 24.0 * eps * (sr6 * sr6 - sr6) / r2                   # [ (s/r)^12 - (s/r)^6 ] / r^2
         f[a:a + chunk] = np.einsum("kj,kja->ka", w, rho)
+    return f
+
+
+def wall_force(pos, lo, hi, eps: float, sigma: float, cutoff: float):
+    """Force of the six walls of the box [lo, hi] on particles inside it.  pos [N][3] -> [N][3], fp64."""
+    p = np.asarray(pos, dtype=np.float64)
+    lo = np.asarray(lo, dtype=np.float64)
+    hi = np.asarray(hi, dtype=np.float64)
+    f = np.zeros_like(p)
+    for a in range(3):
+        for d, sign in ((p[:, a] - lo[a], +1.0), (hi[a] - p[:, a], -1.0)):     # distance to the wall, inward normal
+            d = np.where(d < cutoff, d, np.inf)
+            sr6 = (sigma / d) ** 6
+            f[:, a] += sign * 24.0 * eps * (sr6 * sr6 - sr6) / d
     return f
 
 

@@ -6,7 +6,7 @@ equations of motion it discretises (error O(dtau)).
 """
 import numpy as np
 
-from oracle.md_step import lj_force, md_step
+from oracle.md_step import lj_force, md_step, wall_force
 
 
 # ------------------------------------------------------------------ Eq. 13 ----
@@ -71,6 +71,40 @@ def test_lj_newton_third_law_cutoff_and_invariance():
             if r < 2.5:
                 ref[k] += 24.0 * d / r ** 2 * (r ** -12 - r ** -6)
     assert np.allclose(lj_force(sub, 1.0, 1.0, 2.5), ref, rtol=1e-12, atol=1e-12)
+
+
+# ------------------------------------------------------------------- walls ----
+def test_wall_force_zero_at_sigma_repulsive_inside_and_gradient():
+    lo, hi = np.zeros(3), np.array([10.0, 10.0, 10.0])
+    eps, sg = 0.9, 0.5
+    # one particle near the x = 0 wall only (every other wall beyond the cut-off)
+    for d, sign in ((0.45, +1), (0.5, 0), (0.7, -1)):
+        f = wall_force(np.array([[d, 5.0, 5.0]]), lo, hi, eps, sg, 2.0)
+        assert np.sign(round(f[0, 0], 12)) == sign and f[0, 1] == 0.0 and f[0, 2] == 0.0
+    # mirror image at the opposite wall, and beyond the cut-off nothing
+    f1 = wall_force(np.array([[0.45, 5.0, 5.0], [9.55, 5.0, 5.0], [5.0, 5.0, 5.0]]), lo, hi, eps, sg, 2.0)
+    assert np.isclose(f1[0, 0], -f1[1, 0]) and np.all(f1[2] == 0.0)
+    # minus the gradient of the wall potential U(d) = 2 eps (s/d)^12 - 4 eps (s/d)^6 summed over the six walls
+    def U(x):
+        d = np.concatenate([x - lo, hi - x])
+        return float((2 * eps * (sg / d) ** 12 - 4 * eps * (sg / d) ** 6).sum())
+    x = np.array([0.62, 9.2, 4.0])
+    f = wall_force(x[None, :], lo, hi, eps, sg, 1e9)[0]
+    for a in range(3):
+        e = np.zeros(3)
+        e[a] = 1e-6
+        g = (U(x + e) - U(x - e)) / 2e-6
+        assert abs(f[a] + g) <= 1e-6 * max(1.0, abs(g))
+
+
+def test_wall_force_monolayer_box_centres_the_layer():
+    # the 2.1 R high box of PAPER.md:204 in diameter units: height 1.05, sigma_w = 0.5 (sphere touching a wall)
+    lo, hi = np.array([0.0, 0.0, 0.0]), np.array([50.0, 50.0, 1.05])
+    mid = wall_force(np.array([[25.0, 25.0, 0.525]]), lo, hi, 1.0, 0.5, 2.5)
+    assert abs(mid[0, 2]) <= 1e-12                                  # the two walls cancel at mid height
+    up = wall_force(np.array([[25.0, 25.0, 0.56]]), lo, hi, 1.0, 0.5, 2.5)
+    down = wall_force(np.array([[25.0, 25.0, 0.49]]), lo, hi, 1.0, 0.5, 2.5)
+    assert up[0, 2] < 0.0 < down[0, 2]                              # restoring towards the mid plane
 
 
 # ------------------------------------------------------- Euler-Maruyama step ----
