@@ -168,6 +168,13 @@ typedef struct ff_step_params {
     float noise_d;       /* amplitude multiplying sqrt(dtau) xi in the velocity update (0 = off) */
     float noise_r;       /* same for the angular velocity */
     uint64_t seed;
+    /* container walls (reading Q20): the six planes of the box [wall_lo, wall_hi]
+     * act on a particle at distance d < lj_cutoff with 24 wall_epsilon / d [ (wall_sigma/d)^12 - (wall_sigma/d)^6 ]
+     * along the inward normal.  wall_epsilon = 0 disables the walls; particles must start inside the box. */
+    float wall_lo[3];
+    float wall_hi[3];
+    float wall_epsilon;
+    float wall_sigma;    /* centre-to-wall distance at which the wall force vanishes */
 } ff_step_params;
 
 int ff_step(ff_ctx* ctx, float* pos, float* vel, float* mom, float* angvel, int64_t n,

@@ -139,6 +139,16 @@ ff_k_integrate(int n, float* __restrict__ pos, float* __restrict__ vel, float* _
         h[a] = H[o + a] + p.h_ext[a];
         f[a] = F[o + a] + (fsr ? fsr[o + a] : 0.0f);
     }
+    if (p.wall_epsilon != 0.0f) {
+        // container walls (reading Q20): Eq. 13's pair term at the distance to each plane
+        const float s2 = p.wall_sigma * p.wall_sigma, e24 = 24.0f * p.wall_epsilon;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const float d0 = x[a] - p.wall_lo[a], d1 = p.wall_hi[a] - x[a];
+            if (d0 < p.lj_cutoff) { float i2 = 1.0f / (d0 * d0), s6 = s2 * i2; s6 = s6 * s6 * s6; f[a] += e24 * (s6 * s6 - s6) / d0; }
+            if (d1 < p.lj_cutoff) { float i2 = 1.0f / (d1 * d1), s6 = s2 * i2; s6 = s6 * s6 * s6; f[a] -= e24 * (s6 * s6 - s6) / d1; }
+        }
+    }
     float xi[6] = { 0.f, 0.f, 0.f, 0.f, 0.f, 0.f };
     if (p.noise_d != 0.0f || p.noise_r != 0.0f) {
         ff_gauss2(p.seed, step, (uint64_t)k, 0u, xi[0], xi[1]);
@@ -170,6 +180,7 @@ int ff_launch_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel,
 {
     int n = (int)n64;
     const float* fsr = nullptr;
+    if (p->wall_epsilon != 0.0f && (!(p->lj_cutoff > 0.0f) || !(p->wall_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
     if (p->lj_epsilon != 0.0f) {
         if (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f)) return FF_ERR_INVALID_ARG;
         size_t cells = (size_t)1 << (3 * FF_LJ_MAX_LEVEL);                   // table sized for the deepest level

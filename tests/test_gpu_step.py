@@ -10,7 +10,7 @@ import pytest
 
 import ffgen
 import oracle
-from oracle.md_step import lj_force, md_step
+from oracle.md_step import lj_force, md_step, wall_force
 
 pytestmark = pytest.mark.gpu
 
@@ -42,6 +42,11 @@ def _params(ff, **kw):
     p.noise_d = kw.get("noise_d", 0.0)
     p.noise_r = kw.get("noise_r", 0.0)
     p.seed = kw.get("seed", 0)
+    for a in range(3):
+        p.wall_lo[a] = kw.get("wall_lo", (0.0, 0.0, 0.0))[a]
+        p.wall_hi[a] = kw.get("wall_hi", (0.0, 0.0, 0.0))[a]
+    p.wall_epsilon = kw.get("wall_eps", 0.0)
+    p.wall_sigma = kw.get("wall_sigma", 0.5)
     return p
 
 
@@ -49,6 +54,9 @@ def _oracle_step(x, v, u, w, theta, kw):
     """fp64 step from the fp32 state (x, v, u, w) the GPU started from."""
     H, F, _, _, Q = oracle.barnes_hut(x, u, theta, 32, scale=True)
     fsr = lj_force(x, kw["eps"], kw["sigma"], kw["cutoff"]) if kw.get("eps", 0.0) != 0.0 else None
+    if kw.get("wall_eps", 0.0) != 0.0:
+        fw = wall_force(x, kw["wall_lo"], kw["wall_hi"], kw["wall_eps"], kw["wall_sigma"], kw.get("cutoff", 2.5))
+        fsr = fw if fsr is None else fsr + fw
     out = md_step(x, v, u, w, H, F, kw.get("dtau", 1e-3), kw.get("gamma_d", 0.0), kw.get("gamma_r", 0.0),
                   kw.get("h_ext", (0.0, 0.0, 0.0)), fsr)
     return out, (H, F, Q, fsr)
@@ -166,3 +174,31 @@ def test_thermal_noise_statistics_and_reproducibility(ff):
     dx, dv, du, dw = _dev(x), _dev(z), _dev(u), _dev(z)
     ctx.step(dx, dv, du, dw, p, 6)
     assert not np.array_equal(dv.cpu().numpy(), outs[0][0].astype(np.float32))
+
+
+def test_monolayer_between_walls(ff):
+    """The paper's second container: a 2.1 R = 1.05 d high box holding one layer of particles.
+    Quasi-2D input: the octree degenerates to a quadtree, and the wall forces are large and nearly cancel."""
+    rng = np.random.default_rng(8)
+    n1 = 64
+    g = np.stack(np.meshgrid(np.arange(n1), np.arange(n1), indexing="ij"), -1).reshape(-1, 2).astype(np.float64)
+    xy = 1.3 * g + rng.uniform(-0.12, 0.12, g.shape)                      # centres >= 1.06 apart
+    z = 0.525 + rng.uniform(-0.03, 0.03, len(g))
+    x = np.column_stack([xy, z]).astype(np.float32)
+    N = len(x)
+    u = ffgen.moments_isotropic(N, 2)
+    v = (0.02 * rng.standard_normal((N, 3))).astype(np.float32)
+    w = (0.1 * rng.standard_normal((N, 3))).astype(np.float32)
+    L = float(1.3 * n1)
+    kw = dict(KW, wall_lo=(-1.0, -1.0, 0.0), wall_hi=(L + 1.0, L + 1.0, 1.05), wall_eps=1.0, wall_sigma=0.5)
+    ctx = ff.FFContext(N, 0.5, counters=True)
+    dx, dv, du, dw = _dev(x), _dev(v), _dev(u), _dev(w)
+    ctx.step(dx, dv, du, dw, _params(ff, **kw), 0)
+    after = [t.cpu().numpy() for t in (dx, dv, du, dw)]
+    ref, aux = _oracle_step(x, v, u, w, 0.5, kw)
+    _check_step((x, v, u, w), after, ref, aux, kw)
+    fw = wall_force(x, kw["wall_lo"], kw["wall_hi"], 1.0, 0.5, 2.5)
+    assert np.abs(fw[:, 2]).max() > 1.0                                   # the walls do act
+    # same interaction sets as the oracle on the flat tree
+    cnt = oracle.barnes_hut(x, u, 0.5, 32)[2]
+    assert ctx.counters() == cnt
