@@ -13,7 +13,9 @@
 
 // ---- radix sort geometry (ff_sort.cu) --------------------------------------
 #define FF_SORT_THREADS 256
+#ifndef FF_SORT_ROUNDS
 #define FF_SORT_ROUNDS 8                                   // keys per thread
+#endif
 #define FF_SORT_TILE (FF_SORT_THREADS * FF_SORT_ROUNDS)    // keys per block
 #define FF_RADIX_BITS 8
 #define FF_RADIX 256

@@ -126,6 +126,41 @@ def test_leaf_capacity(ff, nleaf):
     check_hf(H, F, Ho, Fo, Q, TOL_BH)
 
 
+@pytest.mark.parametrize("case", range(12))
+def test_random_sweep_of_theta_leaf_size_and_shape(ff, case):
+    """Seeded sweep over opening angle, leaf capacity, size and spatial structure (uniform hard spheres, chains,
+    a dense blob inside a dilute gas, a thin slab): identical interaction counters (every accept / open / defer
+    decision of the walk's pre-filter agrees with the oracle's exact rule) and H, F within tolerance."""
+    rng = np.random.default_rng(1000 + case)
+    theta = float(rng.choice([0.2, 0.35, 0.5, 0.6, 0.8, 1.0, 1.3]))
+    nleaf = int(rng.choice([1, 1, 1, 3, 16]))
+    N = int(rng.integers(200, 5000))
+    shape = case % 4
+    if shape == 0:
+        c = ffgen.config(1, N=N, seed=case)
+        pos, mom = c["pos"], c["mom"]
+    elif shape == 1:
+        c = ffgen.config(4, N=N, seed=case)
+        pos, mom = c["pos"], c["mom"]
+    elif shape == 2:                       # blob (jittered lattice, spacing 1.05) inside a dilute gas
+        c = ffgen.config(1, N=N, seed=case)
+        g = np.stack(np.meshgrid(*[np.arange(6)] * 3, indexing="ij"), -1).reshape(-1, 3)
+        blob = (1.05 * g + rng.uniform(-0.02, 0.02, g.shape) + 200.0).astype(np.float32)
+        pos = np.vstack([c["pos"], blob]).astype(np.float32)
+        mom = np.vstack([c["mom"], ffgen.moments_isotropic(len(blob), case)]).astype(np.float32)
+    else:                                  # thin slab: quasi-2D tree
+        n1 = int(np.sqrt(N))
+        g = np.stack(np.meshgrid(np.arange(n1), np.arange(n1), indexing="ij"), -1).reshape(-1, 2)
+        xy = 1.2 * g + rng.uniform(-0.08, 0.08, g.shape)
+        pos = np.column_stack([xy, rng.uniform(0.0, 0.05, len(g))]).astype(np.float32)
+        mom = ffgen.moments_isotropic(len(pos), case)
+    ctx, H, F = _gpu_bh(ff, pos, mom, theta, nleaf=nleaf)
+    Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, theta, 32, nleaf=nleaf, scale=True)
+    _check_tree(ff, ctx, otree, otree.moments(mom))
+    assert ctx.counters() == cnt, (theta, nleaf, len(pos), shape)
+    check_hf(H, F, Ho, Fo, Q, TOL_BH)
+
+
 def test_theta_zero_equals_all_pairs(ff):
     c = ffgen.config(1, N=1200, seed=5)
     pos, mom = c["pos"], c["mom"]
