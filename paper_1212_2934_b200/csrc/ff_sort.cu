@@ -262,7 +262,10 @@ int ff_launch_bbox_keys(ff_ctx* c, const float* pos)
     FF_LAUNCH(c, ff_k_reset, 1, FF_SORT_PASSES * FF_RADIX, 0, c->g);
     int blocks = min((n + 255) / 256, c->num_sms * 8);
     FF_LAUNCH(c, ff_k_bbox, blocks, 256, 0, pos, n, c->g);
-    FF_LAUNCH(c, ff_k_keys, blocks, 256, 0, pos, n, c->g, c->key[0], c->sort_status, FF_SORT_PASSES * n_tiles * FF_RADIX);
+    // every block ends with 1024 global atomics (its digit histograms): few blocks while the launch is latency
+    // bound (measured: 2 per SM at 2^20, 8 per SM at 2^24)
+    int kblocks = min((n + 255) / 256, c->num_sms * (n > (1 << 22) ? 8 : 2));
+    FF_LAUNCH(c, ff_k_keys, kblocks, 256, 0, pos, n, c->g, c->key[0], c->sort_status, FF_SORT_PASSES * n_tiles * FF_RADIX);
     return FF_OK;
 }
 
