@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(256) ff_k_keys(const float* __restrict__ pos, 
 __global__ void __launch_bounds__(FF_SORT_THREADS)
 ff_k_radix_onesweep(const uint32_t* __restrict__ kin, const uint32_t* __restrict__ vin,
                     uint32_t* __restrict__ kout, uint32_t* __restrict__ vout, int n, int pass,
-                    uint32_t* status, ff_globals* g)
+                    uint32_t* status, ff_globals* g, const float* __restrict__ pos, float4* __restrict__ pos_s)
 {
     __shared__ uint32_t wh[FF_SORT_THREADS / 32][FF_RADIX];   // per-warp digit counts, then offsets
     __shared__ uint32_t tile_base[FF_RADIX];
@@ -239,20 +239,13 @@ ff_k_radix_onesweep(const uint32_t* __restrict__ kin, const uint32_t* __restrict
         if (i < tile_n) {
             uint32_t k = skey[i];
             uint32_t dst = tile_base[(k >> shift) & (FF_RADIX - 1)] + (uint32_t)i;
+            const uint32_t v = sval[i];
             kout[dst] = k;
-            vout[dst] = sval[i];
+            vout[dst] = v;
+            // last pass: dst is the final sorted slot, so the sorted float4 positions are written here as well
+            if (pos_s) pos_s[dst] = make_float4(__ldg(pos + 3 * (size_t)v), __ldg(pos + 3 * (size_t)v + 1), __ldg(pos + 3 * (size_t)v + 2), 0.0f);
         }
     }
-}
-
-// sorted float4 copy of a caller-order [n][3] array: out[s] = in[perm[s]]
-__global__ void __launch_bounds__(256) ff_k_gather4(const float* __restrict__ in, const uint32_t* __restrict__ perm,
-                                                    int n, float4* __restrict__ out)
-{
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n) return;
-    size_t j = (size_t)__ldg(perm + s) * 3;
-    out[s] = make_float4(__ldg(in + j), __ldg(in + j + 1), __ldg(in + j + 2), 0.0f);
 }
 
 int ff_launch_bbox_keys(ff_ctx* c, const float* pos)
@@ -277,10 +270,11 @@ int ff_launch_sort(ff_ctx* c, const float* pos)
     for (int pass = 0; pass < FF_SORT_PASSES; ++pass) {
         FF_LAUNCH(c, ff_k_radix_onesweep, n_tiles, FF_SORT_THREADS, 0, c->key[cur],
                   pass == 0 ? (const uint32_t*)nullptr : c->idx[cur], c->key[cur ^ 1], c->idx[cur ^ 1], n, pass,
-                  c->sort_status + (size_t)pass * n_tiles * FF_RADIX, c->g);
+                  c->sort_status + (size_t)pass * n_tiles * FF_RADIX, c->g,
+                  pass == FF_SORT_PASSES - 1 ? pos : (const float*)nullptr,
+                  pass == FF_SORT_PASSES - 1 ? c->pos_s : (float4*)nullptr);
         cur ^= 1;
     }
-    // four passes: the result is back in buffer 0
-    FF_LAUNCH(c, ff_k_gather4, (n + 255) / 256, 256, 0, pos, c->idx[0], n, c->pos_s);
+    // four passes: the result is back in buffer 0 (and the sorted positions are in pos_s)
     return FF_OK;
 }
