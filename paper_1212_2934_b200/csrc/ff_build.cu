@@ -253,9 +253,18 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
         const float s2 = __fmul_rn(s, s);
         const int ls = g->level_start[level], le = g->level_start[level + 1];
         const int kstep = solo ? FF_MOM_THREADS / 8 : ngroups;
-        for (int k = ls + (solo ? (int)(threadIdx.x >> 3) : gid); k < le; k += kstep) {
-            const int id = cell_list[k];
-            const int32_t e = cell_child[8 * (size_t)id + o];
+        // software pipeline over the dependent loads list -> child link -> child data: the cell id is fetched two
+        // iterations ahead and the child link one ahead, so that an iteration exposes one memory latency, not three
+        const int k0 = ls + (solo ? (int)(threadIdx.x >> 3) : gid);
+        int id1 = k0 < le ? cell_list[k0] : -1;                        // cell of the coming iteration
+        int id2 = k0 + kstep < le ? cell_list[k0 + kstep] : -1;        // and of the one after
+        int32_t e1 = id1 >= 0 ? cell_child[8 * (size_t)id1 + o] : FF_CHILD_EMPTY;
+        for (int k = k0; k < le; k += kstep) {
+            const int id = id1;
+            const int32_t e = e1;
+            id1 = id2;
+            id2 = k + 2 * kstep < le ? cell_list[k + 2 * kstep] : -1;
+            e1 = id1 >= 0 ? cell_child[8 * (size_t)id1 + o] : FF_CHILD_EMPTY;
             const bool have = e != FF_CHILD_EMPTY;
             if (e >= 0) {
                 // plain loads: written earlier in this launch by other blocks (ordered by grid.sync)
