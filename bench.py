@@ -37,7 +37,7 @@ FLOP_PER_INTERACTION = 60.0      # 21 FFMA x2 + 17 FADD/FMUL + 1 MUFU
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one ff_k_walk launch at config 3, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists)
-WALK_DRAM_TRAFFIC_BYTES = 107017728   # 84.70 MB read + 22.31 MB written (profiles/r1_walk_full.md)
+WALK_DRAM_TRAFFIC_BYTES = 107508480   # 84.74 MB read + 22.76 MB written (profiles/r1_walk_full.md)
 
 
 def _peaks():
