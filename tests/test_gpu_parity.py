@@ -220,6 +220,32 @@ def test_context_reuse_and_smaller_n(ff):
         check_hf(H.cpu().numpy(), F.cpu().numpy(), Ho, Fo, Q, TOL_BH)
 
 
+def test_user_stream_and_repeatability(ff, cfg1):
+    """All work is enqueued on the stream given to ff_set_stream (cooperative launches included) and the
+    result does not depend on the stream or on the run: bit-identical H and F."""
+    import torch
+    pos, mom = _dev(cfg1["pos"]), _dev(cfg1["mom"])
+    ctx = ff.FFContext(len(cfg1["pos"]), 0.5)
+    ctx.build_tree(pos)
+    H0, F0 = ctx.eval_bh(pos, mom)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    ctx.set_stream(side.cuda_stream)
+    with torch.cuda.stream(side):
+        ctx.build_tree(pos)
+        H1, F1 = ctx.eval_bh(pos, mom)
+        Hd, Fd = ctx.eval_direct(pos, mom)
+    side.synchronize()
+    assert torch.equal(H0, H1) and torch.equal(F0, F1)
+    Hh, Fh = np.empty_like(cfg1["pos"]), np.empty_like(cfg1["pos"])
+    ctx.eval_bh_host(cfg1["pos"], cfg1["mom"], Hh, Fh)                 # second stream for the moment upload
+    assert np.array_equal(Hh, H0.cpu().numpy()) and np.array_equal(Fh, F0.cpu().numpy())
+    ctx.set_stream(torch.cuda.current_stream().cuda_stream)
+    H2, F2 = ctx.eval_direct(pos, mom)
+    torch.cuda.synchronize()
+    assert torch.equal(H2, Hd) and torch.equal(F2, Fd)
+
+
 def test_error_codes(ff):
     ctx = ff.FFContext(100, 0.5)
     p = _dev(ffgen.uniform_points(100, 5.0, 0))
