@@ -139,6 +139,17 @@ int ff_eval_direct(ff_ctx* ctx, const float* pos, const float* mom, int64_t n, f
  */
 int ff_eval_bh_host(ff_ctx* ctx, const float* pos_host, const float* mom_host, int64_t n,
                     float* H_host, float* F_host);
+/*
+ * The same without the final synchronise: enqueues upload, ff_build_tree + ff_eval_bh and download and returns.
+ * Uploads, compute and downloads use three streams and two sets of staging buffers, so in a sequence of calls
+ * the copies of one call overlap the compute of its neighbours.  The host buffers must be page-locked for the
+ * copies to be asynchronous and must not be touched (inputs: not modified; outputs: not read) before
+ * ff_host_sync returns.  At most two calls are in flight on the device; a third waits on the GPU, not on the host.
+ */
+int ff_eval_bh_host_async(ff_ctx* ctx, const float* pos_host, const float* mom_host, int64_t n,
+                          float* H_host, float* F_host);
+/* Block until every *_host call issued on this context has delivered its results. */
+int ff_host_sync(ff_ctx* ctx);
 int ff_eval_direct_host(ff_ctx* ctx, const float* pos_host, const float* mom_host, int64_t n,
                         float* H_host, float* F_host);
 

@@ -32,7 +32,7 @@ FF_CHILD_LEAF1, FF_CHILD_MULTI, FF_CHILD_SLOT = 0x80000000, 0x40000000, 0x3FFFFF
 SYMBOLS = (
     "ff_workspace_bytes", "ff_create", "ff_destroy", "ff_set_stream", "ff_set_option", "ff_build_tree",
     "ff_eval_bh", "ff_eval_direct", "ff_eval_bh_host", "ff_eval_direct_host", "ff_step", "ff_get_tree",
-    "ff_get_timings", "ff_get_counters", "ff_get_prefilter_count", "ff_get_launch_count", "ff_measure_fp32_peak", "ff_error_string",
+    "ff_get_timings", "ff_eval_bh_host_async", "ff_host_sync", "ff_get_counters", "ff_get_prefilter_count", "ff_get_launch_count", "ff_measure_fp32_peak", "ff_error_string",
     "ff_last_error",
 )
 
@@ -87,6 +87,10 @@ def lib():
         L.ff_eval_direct.argtypes = [vp, vp, vp, i64, vp, vp]
         L.ff_eval_bh_host.restype = i32
         L.ff_eval_bh_host.argtypes = [vp, vp, vp, i64, vp, vp]
+        L.ff_eval_bh_host_async.restype = i32
+        L.ff_eval_bh_host_async.argtypes = [vp, vp, vp, i64, vp, vp]
+        L.ff_host_sync.restype = i32
+        L.ff_host_sync.argtypes = [vp]
         L.ff_eval_direct_host.restype = i32
         L.ff_eval_direct_host.argtypes = [vp, vp, vp, i64, vp, vp]
         L.ff_step.restype = i32
@@ -228,6 +232,14 @@ class FFContext:
     def eval_bh_host(self, pos, mom, H, F):
         """End to end with HOST buffers (numpy or CPU torch, ideally pinned): H2D, build, eval, D2H."""
         return self._host(self._L.ff_eval_bh_host, "ff_eval_bh_host", pos, mom, H, F)
+
+    def eval_bh_host_async(self, pos, mom, H, F):
+        """eval_bh_host without the final synchronise: successive calls overlap their copies with each other's
+        compute.  Use pinned buffers, keep them alive and untouched until host_sync()."""
+        return self._host(self._L.ff_eval_bh_host_async, "ff_eval_bh_host_async", pos, mom, H, F)
+
+    def host_sync(self):
+        self._check(self._L.ff_host_sync(self._h), "ff_host_sync")
 
     def eval_direct_host(self, pos, mom, H, F):
         return self._host(self._L.ff_eval_direct_host, "ff_eval_direct_host", pos, mom, H, F)

@@ -41,10 +41,13 @@ static size_t carve(ff_ctx* c, char* base, int64_t N)
     p = take(cap * 24);                           if (c) c->cell_sum_u = (double*)p;
     p = take(cap * 24);                           if (c) c->cell_sum_p = (double*)p;
     p = take((size_t)FF_DIRECT_SPLIT_ELEMS * 48); if (c) c->direct_part = (double*)p;
-    p = take(n * 12);                             if (c) c->stage_pos = (float*)p;
-    p = take(n * 12);                             if (c) c->stage_mom = (float*)p;
-    p = take(n * 12);                             if (c) c->stage_H = (float*)p;
-    p = take(n * 12);                             if (c) c->stage_F = (float*)p;
+    for (int b = 0; b < 2; ++b) {
+        p = take(n * 12);                         if (c) c->stage_pos2[b] = (float*)p;
+        p = take(n * 12);                         if (c) c->stage_mom2[b] = (float*)p;
+        p = take(n * 12);                         if (c) c->stage_H2[b] = (float*)p;
+        p = take(n * 12);                         if (c) c->stage_F2[b] = (float*)p;
+    }
+    if (c) { c->stage_H = c->stage_H2[0]; c->stage_F = c->stage_F2[0]; }
     p = take(n * 12);                             if (c) c->step_fsr = (float*)p;
     if (c) c->cell_cap = (int64_t)cap;
     return off;
@@ -73,8 +76,14 @@ extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, 
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
     for (int ph = 0; e == cudaSuccess && ph < FF_N_PHASES; ++ph)
         for (int k = 0; e == cudaSuccess && k < 2; ++k) e = cudaEventCreate(&c->ev[ph][k]);
-    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->copy_done, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->in_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->out_stream, cudaStreamNonBlocking);
+    for (int b = 0; e == cudaSuccess && b < 2; ++b) {
+        e = cudaEventCreateWithFlags(&c->ev_pos[b], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_in[b], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_done[b], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_out[b], cudaEventDisableTiming);
+    }
     if (e == cudaSuccess) e = cudaMemset(c->g, 0, sizeof(ff_globals));
     if (e != cudaSuccess) { delete c; return FF_ERR_CUDA; }
     *out = c;
@@ -87,8 +96,16 @@ extern "C" int ff_destroy(ff_ctx* c)
     cudaStreamSynchronize(c->stream);
     for (int ph = 0; ph < FF_N_PHASES; ++ph)
         for (int k = 0; k < 2; ++k) if (c->ev[ph][k]) cudaEventDestroy(c->ev[ph][k]);
-    if (c->copy_done) cudaEventDestroy(c->copy_done);
-    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->in_stream) cudaStreamSynchronize(c->in_stream);
+    if (c->out_stream) cudaStreamSynchronize(c->out_stream);
+    for (int b = 0; b < 2; ++b) {
+        if (c->ev_pos[b]) cudaEventDestroy(c->ev_pos[b]);
+        if (c->ev_in[b]) cudaEventDestroy(c->ev_in[b]);
+        if (c->ev_done[b]) cudaEventDestroy(c->ev_done[b]);
+        if (c->ev_out[b]) cudaEventDestroy(c->ev_out[b]);
+    }
+    if (c->in_stream) cudaStreamDestroy(c->in_stream);
+    if (c->out_stream) cudaStreamDestroy(c->out_stream);
     delete c;
     return FF_OK;
 }
@@ -164,38 +181,71 @@ extern "C" int ff_eval_direct(ff_ctx* c, const float* pos, const float* mom, int
     return FF_OK;
 }
 
-static int host_roundtrip(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h, bool bh)
+// ---- *_host calls: uploads, compute and downloads on three streams, double-buffered by call parity ----
+// Call i uses staging buffer b = i & 1.  Ordering (events, no host waits):
+//   in_stream   wait ev_done[b] (call i-2 has finished reading buffer b) ; H2D pos -> ev_pos[b] ; H2D mom -> ev_in[b]
+//   stream      wait ev_pos[b] ; tree build ; wait ev_in[b] ; wait ev_out[b] (call i-2's download has left the
+//               result buffer) ; moments + walk (or the all-pairs kernel) -> ev_done[b]
+//   out_stream  wait ev_done[b] ; D2H H, F -> ev_out[b]
+// so that in a sequence of calls the copies of one call run under the compute of its neighbours (PCIe is full
+// duplex), and inside one call the moment upload runs under the tree build.
+static int host_enqueue(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h, bool bh)
 {
     if (!c || !pos_h || !mom_h || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
-    size_t bytes = (size_t)n * 12;
-    FF_CUDA(c, cudaMemcpyAsync(c->stage_pos, pos_h, bytes, cudaMemcpyHostToDevice, c->stream));
+    const int b = (int)(c->host_seq & 1);
+    const size_t bytes = (size_t)n * 12;
+    FF_CUDA(c, cudaStreamWaitEvent(c->in_stream, c->ev_done[b], 0));
+    FF_CUDA(c, cudaMemcpyAsync(c->stage_pos2[b], pos_h, bytes, cudaMemcpyHostToDevice, c->in_stream));
+    FF_CUDA(c, cudaEventRecord(c->ev_pos[b], c->in_stream));
+    FF_CUDA(c, cudaMemcpyAsync(c->stage_mom2[b], mom_h, bytes, cudaMemcpyHostToDevice, c->in_stream));
+    FF_CUDA(c, cudaEventRecord(c->ev_in[b], c->in_stream));
+    float* Hd = H_h ? c->stage_H2[b] : nullptr;
+    float* Fd = F_h ? c->stage_F2[b] : nullptr;
     int rc;
+    FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_pos[b], 0));
     if (bh) {
-        // the moments are not needed before the cell sums: their copy runs on a second stream under the
-        // tree build (the previous call ended with a stream synchronise, so stage_mom is free)
-        FF_CUDA(c, cudaMemcpyAsync(c->stage_mom, mom_h, bytes, cudaMemcpyHostToDevice, c->copy_stream));
-        FF_CUDA(c, cudaEventRecord(c->copy_done, c->copy_stream));
-        if ((rc = ff_build_tree(c, c->stage_pos, n)) != FF_OK) return rc;
-        FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->copy_done, 0));
-        if ((rc = ff_eval_bh(c, c->stage_pos, c->stage_mom, H_h ? c->stage_H : nullptr, F_h ? c->stage_F : nullptr)) != FF_OK) return rc;
+        if ((rc = ff_build_tree(c, c->stage_pos2[b], n)) != FF_OK) return rc;
+        FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[b], 0));
+        FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[b], 0));
+        if ((rc = ff_eval_bh(c, c->stage_pos2[b], c->stage_mom2[b], Hd, Fd)) != FF_OK) return rc;
     } else {
-        FF_CUDA(c, cudaMemcpyAsync(c->stage_mom, mom_h, bytes, cudaMemcpyHostToDevice, c->stream));
-        if ((rc = ff_eval_direct(c, c->stage_pos, c->stage_mom, n, H_h ? c->stage_H : nullptr, F_h ? c->stage_F : nullptr)) != FF_OK) return rc;
+        FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[b], 0));
+        FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[b], 0));
+        if ((rc = ff_eval_direct(c, c->stage_pos2[b], c->stage_mom2[b], n, Hd, Fd)) != FF_OK) return rc;
     }
-    if (H_h) FF_CUDA(c, cudaMemcpyAsync(H_h, c->stage_H, bytes, cudaMemcpyDeviceToHost, c->stream));
-    if (F_h) FF_CUDA(c, cudaMemcpyAsync(F_h, c->stage_F, bytes, cudaMemcpyDeviceToHost, c->stream));
-    FF_CUDA(c, cudaStreamSynchronize(c->stream));
+    FF_CUDA(c, cudaEventRecord(c->ev_done[b], c->stream));
+    FF_CUDA(c, cudaStreamWaitEvent(c->out_stream, c->ev_done[b], 0));
+    if (H_h) FF_CUDA(c, cudaMemcpyAsync(H_h, Hd, bytes, cudaMemcpyDeviceToHost, c->out_stream));
+    if (F_h) FF_CUDA(c, cudaMemcpyAsync(F_h, Fd, bytes, cudaMemcpyDeviceToHost, c->out_stream));
+    FF_CUDA(c, cudaEventRecord(c->ev_out[b], c->out_stream));
+    c->host_seq++;
     return FF_OK;
+}
+
+extern "C" int ff_host_sync(ff_ctx* c)
+{
+    if (!c) return FF_ERR_INVALID_ARG;
+    FF_CUDA(c, cudaStreamSynchronize(c->in_stream));
+    FF_CUDA(c, cudaStreamSynchronize(c->stream));
+    FF_CUDA(c, cudaStreamSynchronize(c->out_stream));
+    return FF_OK;
+}
+
+extern "C" int ff_eval_bh_host_async(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h)
+{
+    return host_enqueue(c, pos_h, mom_h, n, H_h, F_h, true);
 }
 
 extern "C" int ff_eval_bh_host(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h)
 {
-    return host_roundtrip(c, pos_h, mom_h, n, H_h, F_h, true);
+    int rc = host_enqueue(c, pos_h, mom_h, n, H_h, F_h, true);
+    return rc != FF_OK ? rc : ff_host_sync(c);
 }
 
 extern "C" int ff_eval_direct_host(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h)
 {
-    return host_roundtrip(c, pos_h, mom_h, n, H_h, F_h, false);
+    int rc = host_enqueue(c, pos_h, mom_h, n, H_h, F_h, false);
+    return rc != FF_OK ? rc : ff_host_sync(c);
 }
 
 extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n,
@@ -205,6 +255,7 @@ extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* ang
     if (!(p->dtau > 0.0f)) return FF_ERR_INVALID_ARG;
     int rc;
     if ((rc = ff_build_tree(c, pos, n)) != FF_OK) return rc;
+    FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[0], 0));   // a pending download of an earlier *_host_async call
     if ((rc = ff_eval_bh(c, pos, mom, c->stage_H, c->stage_F)) != FF_OK) return rc;
     ff_phase_begin(c, FF_PH_STEP);
     if ((rc = ff_launch_step(c, pos, vel, mom, angvel, n, p, step_index)) != FF_OK) return rc;

@@ -76,8 +76,11 @@ struct ff_ctx {
     int device;
     int num_sms;
     cudaStream_t stream;
-    cudaStream_t copy_stream;         // second stream of the *_host calls (moment upload under the tree build)
-    cudaEvent_t copy_done;
+    // pipelined *_host calls: uploads on in_stream, compute on `stream`, downloads on out_stream, staging
+    // buffers and events double-buffered by call parity (ff_api.cu)
+    cudaStream_t in_stream, out_stream;
+    cudaEvent_t ev_pos[2], ev_in[2], ev_done[2], ev_out[2];
+    uint64_t host_seq;                // *_host calls issued so far
     uint64_t launches;
     char last_error[256];
 
@@ -96,7 +99,8 @@ struct ff_ctx {
     float4 *cell_centre, *cell_moment;
     double *cell_sum_u, *cell_sum_p;  // [cap][3] fp64 sums in the fixed order
     double* direct_part;              // partial sums of the split direct kernel
-    float *stage_pos, *stage_mom, *stage_H, *stage_F;   // device staging of the *_host calls / ff_step fields
+    float *stage_pos2[2], *stage_mom2[2], *stage_H2[2], *stage_F2[2];   // device staging of the *_host calls
+    float *stage_H, *stage_F;         // = stage_H2[0], stage_F2[0]: the fields of ff_step
     float* step_fsr;                  // [N][3] short-range force (ff_step)
 
     cudaEvent_t ev[FF_N_PHASES][2];

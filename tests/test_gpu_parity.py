@@ -246,6 +246,33 @@ def test_user_stream_and_repeatability(ff, cfg1):
     assert torch.equal(H2, Hd) and torch.equal(F2, Fd)
 
 
+def test_pipelined_host_calls(ff):
+    """ff_eval_bh_host_async: several calls in flight with different inputs, two result buffers per call parity;
+    every result equals the synchronous call's, bit for bit."""
+    import torch
+    sets = [ffgen.config(1, N=n, seed=s) for n, s in ((4096, 1), (3000, 2), (4096, 3), (1777, 4), (4096, 5))]
+    ctx = ff.FFContext(4096, 0.5)
+    ref = []
+    for c in sets:
+        H, F = np.empty_like(c["pos"]), np.empty_like(c["pos"])
+        ctx.eval_bh_host(c["pos"], c["mom"], H, F)
+        ref.append((H.copy(), F.copy()))
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    ins = [(pin(c["pos"]), pin(c["mom"])) for c in sets]
+    outs = [(torch.empty(c["pos"].shape, dtype=torch.float32).pin_memory(),
+             torch.empty(c["pos"].shape, dtype=torch.float32).pin_memory()) for c in sets]
+    for (p, m), (H, F) in zip(ins, outs):
+        ctx.eval_bh_host_async(p, m, H, F)
+    ctx.host_sync()
+    for (H, F), (Hr, Fr) in zip(outs, ref):
+        assert np.array_equal(H.numpy(), Hr) and np.array_equal(F.numpy(), Fr)
+    # a device-side call and ff_step after pipelined calls see a consistent context
+    c = sets[0]
+    ctx.build_tree(_dev(c["pos"]))
+    H, F = ctx.eval_bh(_dev(c["pos"]), _dev(c["mom"]))
+    assert np.array_equal(H.cpu().numpy(), ref[0][0])
+
+
 def test_error_codes(ff):
     ctx = ff.FFContext(100, 0.5)
     p = _dev(ffgen.uniform_points(100, 5.0, 0))
