@@ -38,8 +38,7 @@ static size_t carve(ff_ctx* c, char* base, int64_t N)
     p = take(cap * 32);                           if (c) c->cell_child = (int32_t*)p;
     p = take(cap * 16);                           if (c) c->cell_centre = (float4*)p;
     p = take(cap * 16);                           if (c) c->cell_moment = (float4*)p;
-    p = take(cap * 24);                           if (c) c->cell_sum_u = (double*)p;
-    p = take(cap * 24);                           if (c) c->cell_sum_p = (double*)p;
+    p = take(cap * 64);                           if (c) c->cell_sums = (double*)p;
     p = take((size_t)FF_DIRECT_SPLIT_ELEMS * 48); if (c) c->direct_part = (double*)p;
     for (int b = 0; b < 2; ++b) {
         p = take(n * 12);                         if (c) c->stage_pos2[b] = (float*)p;

@@ -222,7 +222,7 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
              const int32_t* __restrict__ cell_first, const int32_t* __restrict__ cell_end,
              const int32_t* __restrict__ cell_list, const int32_t* __restrict__ cell_child,
              const int32_t* __restrict__ leaf_count, const float4* __restrict__ pos_s, float4* __restrict__ mom_s,
-             double* __restrict__ sum_u, double* __restrict__ sum_p, float4* __restrict__ centre,
+             double* __restrict__ sums, float4* __restrict__ centre,
              float4* __restrict__ moment)
 {
     cg::grid_group grid = cg::this_grid();
@@ -269,7 +269,10 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
             if (e >= 0) {
                 // plain loads: written earlier in this launch by other blocks (ordered by grid.sync)
 #pragma unroll
-                for (int a = 0; a < 3; ++a) { mine[o][a] = sum_u[3 * (size_t)e + a]; mine[o][3 + a] = sum_p[3 * (size_t)e + a]; }
+                for (int a = 0; a < 6; a += 2) {           // one 64-byte record per cell: u.xyz, p.xyz (two sectors)
+                    const double2 v = *reinterpret_cast<const double2*>(sums + 8 * (size_t)e + a);
+                    mine[o][a] = v.x; mine[o][a + 1] = v.y;
+                }
             } else if (have) {
                 int slot = (int)((uint32_t)e & FF_CHILD_SLOT);
                 int cc = ((uint32_t)e & FF_CHILD_MULTI) ? leaf_count[slot] : 1;
@@ -291,7 +294,7 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
 #pragma unroll
                 for (int c = 0; c < 8; ++c)
                     if (present & (1u << c)) { t = started ? t + mine[c][o] : mine[c][o]; started = true; }
-                if (o < 3) sum_u[3 * (size_t)id + o] = t; else sum_p[3 * (size_t)id + (o - 3)] = t;
+                sums[8 * (size_t)id + o] = t;
             }
             float* cen = reinterpret_cast<float*>(centre + id);
             float* mo = reinterpret_cast<float*>(moment + id);
@@ -338,7 +341,7 @@ int ff_launch_moments(ff_ctx* c, const float* mom)
     const uint32_t* perm = c->idx[0];
     void* args[] = { (void*)&mom, (void*)&perm, (void*)&n, (void*)&c->g, (void*)&c->cell_first, (void*)&c->cell_end,
                      (void*)&c->cell_list, (void*)&c->cell_child, (void*)&c->leaf_count, (void*)&c->pos_s,
-                     (void*)&c->mom_s, (void*)&c->cell_sum_u, (void*)&c->cell_sum_p, (void*)&c->cell_centre,
+                     (void*)&c->mom_s, (void*)&c->cell_sums, (void*)&c->cell_centre,
                      (void*)&c->cell_moment };
     FF_CUDA(c, cudaLaunchCooperativeKernel((const void*)ff_k_moments, dim3(blocks), dim3(FF_MOM_THREADS), args, 0,
                                            c->stream));

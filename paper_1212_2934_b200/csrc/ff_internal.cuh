@@ -97,7 +97,7 @@ struct ff_ctx {
     int32_t* cell_list;               // [cap] cell ids grouped by level
     int32_t* cell_child;              // [cap][8]
     float4 *cell_centre, *cell_moment;
-    double *cell_sum_u, *cell_sum_p;  // [cap][3] fp64 sums in the fixed order
+    double* cell_sums;                // [cap][8] fp64 sums in the fixed order: u.xyz, p.xyz, 2 pad (64-byte records)
     double* direct_part;              // partial sums of the split direct kernel
     float *stage_pos2[2], *stage_mom2[2], *stage_H2[2], *stage_F2[2];   // device staging of the *_host calls
     float *stage_H, *stage_F;         // = stage_H2[0], stage_F2[0]: the fields of ff_step
