@@ -337,6 +337,23 @@ def run_ours(args):
                                 "tflops": pairs * FLOP_PER_INTERACTION / (d_ms * 1e-3) / 1e12,
                                 "frac_of_fp32_peak": pairs * FLOP_PER_INTERACTION / (d_ms * 1e-3) / 1e12 / peak_tflops,
                                 "flop_per_pair": FLOP_PER_INTERACTION, "speedup_bh_over_direct": d_ms / ms_per_step}
+        # the oracle's all-pairs sum on a sample of targets (all sources), on the host cores: the GPU result of those
+        # targets is checked against it, and its rate extrapolated to all N targets is the CPU all-pairs baseline
+        # the paper's Table 1 compares with (there: one core, single precision)
+        import oracle as _oracle
+        rng = np.random.default_rng(1)
+        tsel = np.sort(rng.choice(N, size=min(N, 1024), replace=False)).astype(np.int64)
+        t0 = time.perf_counter()
+        Ha, Fa, Qa = _oracle.allpairs(c["pos"], c["mom"], targets=tsel, scale=True)
+        t_ap = time.perf_counter() - t0
+        Hs, Fs = Hd[torch.from_numpy(tsel).to(dev)].cpu().numpy(), Fd[torch.from_numpy(tsel).to(dev)].cpu().numpy()
+        eH = float((np.linalg.norm(Hs - Ha, axis=1) / np.maximum(np.linalg.norm(Ha, axis=1), Qa[:, 0] / 8)).max())
+        eF = float((np.linalg.norm(Fs - Fa, axis=1) / np.maximum(np.linalg.norm(Fa, axis=1), Qa[:, 1] / 8)).max())
+        extras["gpu_direct"].update({
+            "max_err_vs_oracle_allpairs": {"H": eH, "F": eF, "targets": int(len(tsel)), "tolerance": 1e-5},
+            "cpu_allpairs_oracle": {"pairs_per_s": len(tsel) * (N - 1) / t_ap, "cores": _oracle.max_threads(),
+                                    "extrapolated_s_per_eval": t_ap * N / len(tsel),
+                                    "sample": "%d targets x all sources, fp64" % len(tsel)}})
         errs = {}
         for th in (0.3, 0.5, 0.7):
             ctx.set_option(ff.FF_OPT_THETA, th)
