@@ -278,7 +278,16 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
         append(take, A, B);
         int4 c0 = make_int4(-1, -1, -1, -1), c1 = c0;
         if (open) { c0 = __ldg(cell_child + 2 * (size_t)e); c1 = __ldg(cell_child + 2 * (size_t)e + 1); }
+        const int lcnt = is_multi ? __ldg(leaf_count + slot) : 0;
         drain();                                           // overlaps the child loads
+        // a bucket leaf of up to eight particles (N_leaf > 1) is expanded like an opened cell: its particles go
+        // back on the stack as single-particle entries and are handled 32 at a time in the coming rounds
+        const bool small_leaf = is_multi && lcnt <= 8;
+        if (small_leaf) {
+            const int32_t p0 = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)slot);
+            c0 = make_int4(p0, lcnt > 1 ? p0 + 1 : -1, lcnt > 2 ? p0 + 2 : -1, lcnt > 3 ? p0 + 3 : -1);
+            c1 = make_int4(lcnt > 4 ? p0 + 4 : -1, lcnt > 5 ? p0 + 5 : -1, lcnt > 6 ? p0 + 6 : -1, lcnt > 7 ? p0 + 7 : -1);
+        }
         // push the children of the opened cells
         int nch = (c0.x != -1) + (c0.y != -1) + (c0.z != -1) + (c0.w != -1) + (c1.x != -1) + (c1.y != -1) +
                   (c1.z != -1) + (c1.w != -1);
@@ -299,12 +308,11 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
         }
         sp_top += total;
         // multi-particle leaves met this round
-        unsigned mm = __ballot_sync(FF_FULL, is_multi);
+        unsigned mm = __ballot_sync(FF_FULL, is_multi && !small_leaf);
         while (mm) {
             int src = __ffs(mm) - 1;
             mm &= mm - 1;
-            int s0 = __shfl_sync(FF_FULL, slot, src);
-            coop_leaf(s0, __ldg(leaf_count + s0));
+            coop_leaf(__shfl_sync(FF_FULL, slot, src), __shfl_sync(FF_FULL, lcnt, src));
         }
         __syncwarp();
     }
