@@ -312,7 +312,7 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
 int ff_launch_build(ff_ctx* c)
 {
     int n = (int)c->n;
-    static int per_sm = 0;
+    int& per_sm = c->occ_build;                            // per context: contexts may live on different devices
     if (!per_sm) {
         FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_build, FF_BUILD_THREADS, 0));
         if (per_sm < 1) return FF_ERR_CUDA;
@@ -332,7 +332,7 @@ int ff_launch_build(ff_ctx* c)
 int ff_launch_moments(ff_ctx* c, const float* mom)
 {
     int n = (int)c->n;
-    static int per_sm = 0;
+    int& per_sm = c->occ_moments;
     if (!per_sm) {
         FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_moments, FF_MOM_THREADS, 0));
         if (per_sm < 1) return FF_ERR_CUDA;

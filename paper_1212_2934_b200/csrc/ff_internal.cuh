@@ -75,6 +75,7 @@ struct ff_ctx {
     int moments_valid;
     int device;
     int num_sms;
+    int occ_walk[2], occ_build, occ_moments;   // resident blocks per SM of the persistent / cooperative kernels (0 = not queried yet)
     cudaStream_t stream;
     // pipelined *_host calls: uploads on in_stream, compute on `stream`, downloads on out_stream, staging
     // buffers and events double-buffered by call parity (ff_api.cu)

@@ -385,7 +385,7 @@ int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out)
     int n = (int)c->n;
     int groups = (n + 31) / 32;
     size_t smem = sizeof(ff_walk_smem) * FF_WALK_WARPS;
-    static int per_sm[2] = { 0, 0 };
+    int* per_sm = c->occ_walk;                             // per context: contexts may live on different devices
     if (!per_sm[0]) {
         FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
