@@ -363,6 +363,25 @@ def run_ours(args):
         ctx.set_option(ff.FF_OPT_THETA, theta)
         extras["bh_vs_allpairs_error"] = {"reference": "GPU direct kernel (ff_eval_direct)", "by_theta": errs}
 
+        # the same recipe at smaller sizes (device-resident, L2 not flushed): how the step scales with N
+        sweep = {}
+        for n_small in (1 << 14, 1 << 16, 1 << 18):
+            if n_small >= N:
+                continue
+            cs = _workload(n_small, rank, args.config)
+            ps, ms_ = torch.from_numpy(cs["pos"]).to(dev), torch.from_numpy(cs["mom"]).to(dev)
+            cx = ff.FFContext(n_small, theta, device=dev)
+            for _ in range(3):
+                cx.build_tree(ps); cx.eval_bh(ps, ms_)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(10):
+                cx.build_tree(ps); cx.eval_bh(ps, ms_)
+            b.record(); b.synchronize()
+            sweep[str(n_small)] = {"ms_per_step": a.elapsed_time(b) / 10, "particle_evals_per_s": n_small / (a.elapsed_time(b) / 10 * 1e-3)}
+            del cx
+        extras["size_sweep"] = sweep
+
         # config 3 as BASELINE.json states it: 100 MD steps (ff_step: tree rebuilt, H and F by Barnes-Hut,
         # Lennard-Jones force, Euler-Maruyama update, dtau = 0.001 as in PAPER.md:200), per-phase timing
         prm = ff.ff_step_params()
