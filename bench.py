@@ -365,7 +365,7 @@ def run_ours(args):
 
         # the same recipe at smaller sizes (device-resident, L2 not flushed): how the step scales with N
         sweep = {}
-        for n_small in (1 << 14, 1 << 16, 1 << 18):
+        for n_small in (1 << 10, 1 << 12, 1 << 14, 1 << 16, 1 << 18):
             if n_small >= N:
                 continue
             cs = _workload(n_small, rank, args.config)
@@ -378,8 +378,16 @@ def run_ours(args):
             for _ in range(10):
                 cx.build_tree(ps); cx.eval_bh(ps, ms_)
             b.record(); b.synchronize()
-            sweep[str(n_small)] = {"ms_per_step": a.elapsed_time(b) / 10, "particle_evals_per_s": n_small / (a.elapsed_time(b) / 10 * 1e-3)}
+            bh_ms = a.elapsed_time(b) / 10
+            cx.eval_direct(ps, ms_)
+            a.record()
+            for _ in range(3):
+                cx.eval_direct(ps, ms_)
+            b.record(); b.synchronize()
+            sweep[str(n_small)] = {"bh_ms_per_step": bh_ms, "allpairs_ms_per_eval": a.elapsed_time(b) / 3,
+                                   "particle_evals_per_s": n_small / (bh_ms * 1e-3)}
             del cx
+        # the paper's Table 1 has the same crossover: all-pairs wins for N ~ 10^3, Barnes-Hut above
         extras["size_sweep"] = sweep
 
         # config 3 as BASELINE.json states it: 100 MD steps (ff_step: tree rebuilt, H and F by Barnes-Hut,
