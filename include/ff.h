@@ -60,7 +60,9 @@ enum {
     FF_OPT_THETA = 1,     /* opening parameter theta >= 0 ("large enough": s/d < theta) */
     FF_OPT_NLEAF = 2,     /* leaf capacity N_leaf >= 1; 1 = the paper's tree. Invalidates the tree. */
     FF_OPT_COUNTERS = 3,  /* != 0: the walk also counts interactions (slower); read with ff_get_counters */
-    FF_OPT_TIMING = 4     /* != 0: record CUDA events around each phase; read with ff_get_timings */
+    FF_OPT_TIMING = 4,    /* != 0: record CUDA events around each phase; read with ff_get_timings */
+    FF_OPT_GROUP = 5      /* targets per walk group W (reading Q2).  The GPU walk implements W = 32, one
+                             warp per group; any other value is FF_ERR_INVALID_ARG (the oracle takes any W) */
 };
 
 /* phases reported by ff_get_timings, in launch order */

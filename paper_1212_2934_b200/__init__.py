@@ -22,7 +22,7 @@ _lib = None
 
 FF_OK = 0
 FF_ERR_INVALID_ARG, FF_ERR_WORKSPACE, FF_ERR_NO_TREE, FF_ERR_CAPACITY, FF_ERR_CUDA = -1, -2, -3, -4, -5
-FF_OPT_THETA, FF_OPT_NLEAF, FF_OPT_COUNTERS, FF_OPT_TIMING = 1, 2, 3, 4
+FF_OPT_THETA, FF_OPT_NLEAF, FF_OPT_COUNTERS, FF_OPT_TIMING, FF_OPT_GROUP = 1, 2, 3, 4, 5
 FF_N_PHASES = 7
 PHASES = ("bbox_keys", "sort", "build", "moments", "walk", "direct", "step")
 FF_CHILD_EMPTY = -1

@@ -131,6 +131,7 @@ extern "C" int ff_set_option(ff_ctx* c, int key, double value)
         return FF_OK;
     case FF_OPT_COUNTERS: c->count_enabled = value != 0.0; return FF_OK;
     case FF_OPT_TIMING: c->timing_enabled = value != 0.0; return FF_OK;
+    case FF_OPT_GROUP: return value == 32.0 ? FF_OK : FF_ERR_INVALID_ARG;
     default: return FF_ERR_INVALID_ARG;
     }
 }

@@ -286,6 +286,9 @@ def test_error_codes(ff):
         ctx.set_option(ff.FF_OPT_THETA, -1.0)
     with pytest.raises(ff.FFError):
         ctx.set_option(99, 1.0)
+    ctx.set_option(ff.FF_OPT_GROUP, 32)                                     # the one group width the GPU walk has
+    with pytest.raises(ff.FFError):
+        ctx.set_option(ff.FF_OPT_GROUP, 16)
 
 
 # ---------------------------------------------------------------- config 2 ----
