@@ -384,8 +384,25 @@ def run_ours(args):
             for _ in range(3):
                 cx.eval_direct(ps, ms_)
             b.record(); b.synchronize()
-            sweep[str(n_small)] = {"bh_ms_per_step": bh_ms, "allpairs_ms_per_eval": a.elapsed_time(b) / 3,
-                                   "particle_evals_per_s": n_small / (bh_ms * 1e-3)}
+            ap_ms = a.elapsed_time(b) / 3
+            # one MD step (ff_step: fields + Lennard-Jones + Euler-Maruyama) with either algorithm
+            md = {}
+            for name, flag in (("md_step_bh_ms", 0), ("md_step_allpairs_ms", 1)):
+                q = ff.ff_step_params()
+                q.dtau, q.gamma_d, q.gamma_r = 1e-3, 1.0, 1.0
+                q.lj_epsilon, q.lj_sigma, q.lj_cutoff = 1.0, 1.0, 2.5
+                q.all_pairs = flag
+                xs, us = ps.clone(), ms_.clone()
+                vs, ws = torch.zeros_like(ps), torch.zeros_like(ps)
+                cx.step(xs, vs, us, ws, q, 0)
+                reps = 10 if (flag == 0 or n_small <= (1 << 16)) else 2
+                a.record()
+                for r in range(reps):
+                    cx.step(xs, vs, us, ws, q, 1 + r)
+                b.record(); b.synchronize()
+                md[name] = a.elapsed_time(b) / reps
+            sweep[str(n_small)] = {"bh_ms_per_step": bh_ms, "allpairs_ms_per_eval": ap_ms,
+                                   "particle_evals_per_s": n_small / (bh_ms * 1e-3), **md}
             del cx
         # the paper's Table 1 has the same crossover: all-pairs wins for N ~ 10^3, Barnes-Hut above
         extras["size_sweep"] = sweep

@@ -188,6 +188,9 @@ typedef struct ff_step_params {
     float wall_hi[3];
     float wall_epsilon;
     float wall_sigma;    /* centre-to-wall distance at which the wall force vanishes */
+    int32_t all_pairs;   /* != 0: h^dip, f^dip and f^sr by the exact all-pairs sum (the paper's Algorithm 1; no tree).
+                            The faster choice below N ~ 10^4 */
+    int32_t reserved;    /* 0 */
 } ff_step_params;
 
 int ff_step(ff_ctx* ctx, float* pos, float* vel, float* mom, float* angvel, int64_t n,

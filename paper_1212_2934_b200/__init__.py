@@ -42,7 +42,8 @@ class ff_step_params(ctypes.Structure):
                 ("h_ext", ctypes.c_float * 3), ("lj_epsilon", ctypes.c_float), ("lj_sigma", ctypes.c_float),
                 ("lj_cutoff", ctypes.c_float), ("noise_d", ctypes.c_float), ("noise_r", ctypes.c_float),
                 ("seed", ctypes.c_uint64), ("wall_lo", ctypes.c_float * 3), ("wall_hi", ctypes.c_float * 3),
-                ("wall_epsilon", ctypes.c_float), ("wall_sigma", ctypes.c_float)]
+                ("wall_epsilon", ctypes.c_float), ("wall_sigma", ctypes.c_float),
+                ("all_pairs", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 class ff_tree_view(ctypes.Structure):

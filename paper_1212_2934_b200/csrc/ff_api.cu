@@ -254,8 +254,24 @@ extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* ang
     if (!c || !pos || !vel || !mom || !angvel || !p || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
     if (!(p->dtau > 0.0f)) return FF_ERR_INVALID_ARG;
     int rc;
-    if ((rc = ff_build_tree(c, pos, n)) != FF_OK) return rc;
     FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[0], 0));   // a pending download of an earlier *_host_async call
+    if (p->all_pairs) {
+        // the paper's All-Pairs step (Algorithm 1): h^dip, f^dip and f^sr in one pair loop, no tree
+        if (p->lj_epsilon != 0.0f && (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
+        c->n = n;
+        ff_phase_begin(c, FF_PH_DIRECT);
+        if ((rc = ff_launch_direct(c, pos, mom, n, c->stage_H, c->stage_F, p->lj_epsilon, p->lj_sigma, p->lj_cutoff)) != FF_OK)
+            return rc;
+        ff_phase_end(c, FF_PH_DIRECT);
+        ff_step_params q = *p;
+        q.lj_epsilon = 0.0f;                                       // already inside stage_F
+        ff_phase_begin(c, FF_PH_STEP);
+        if ((rc = ff_launch_step(c, pos, vel, mom, angvel, n, &q, step_index)) != FF_OK) return rc;
+        ff_phase_end(c, FF_PH_STEP);
+        c->tree_built = 0;
+        return FF_OK;
+    }
+    if ((rc = ff_build_tree(c, pos, n)) != FF_OK) return rc;
     if ((rc = ff_eval_bh(c, pos, mom, c->stage_H, c->stage_F)) != FF_OK) return rc;
     ff_phase_begin(c, FF_PH_STEP);
     if ((rc = ff_launch_step(c, pos, vel, mom, angvel, n, p, step_index)) != FF_OK) return rc;

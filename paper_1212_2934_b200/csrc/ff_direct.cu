@@ -23,9 +23,25 @@ __device__ __forceinline__ float2 ff_rsqrt2(float2 r2) { return make_float2(ff_r
 #ifndef FF_DIRECT_MINB
 #define FF_DIRECT_MINB 2      // lets ptxas use 92 registers (2 x 8 warps per SM): measured 3 % faster than 66 or 64
 #endif
+// Lennard-Jones coefficient of Eq. 13 for two sources: w = 24 eps [ (s/r)^12 - (s/r)^6 ] / r^2 inside the cut-off,
+// 0 outside and for a masked term (rinv = 0)
+struct ff_lj { float e24, s2, rc2; };
+__device__ __forceinline__ float2 ff_lj2(float2 r2, float2 rinv, const ff_lj& lj)
+{
+    const float2 i2 = __fmul2_rn(rinv, rinv);
+    const float2 sr2 = __fmul2_rn(i2, ff_dup(lj.s2));
+    const float2 sr6 = __fmul2_rn(__fmul2_rn(sr2, sr2), sr2);
+    const float2 t = __ffma2_rn(sr6, sr6, make_float2(-sr6.x, -sr6.y));
+    const float2 w = __fmul2_rn(t, __fmul2_rn(i2, ff_dup(lj.e24)));
+    return make_float2(r2.x < lj.rc2 ? w.x : 0.0f, r2.y < lj.rc2 ? w.y : 0.0f);
+}
+
+// LJ = true: the all-pairs MD step of the paper (Algorithm 1 sums f^dip, f^sr and h^dip in one loop): F_out gets
+// f^dip + f^sr.
+template <bool LJ>
 __global__ void __launch_bounds__(FF_DIRECT_THREADS, FF_DIRECT_MINB)
 ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n, int splits,
-            double* __restrict__ part, float* __restrict__ H_out, float* __restrict__ F_out)
+            double* __restrict__ part, float* __restrict__ H_out, float* __restrict__ F_out, ff_lj lj)
 {
     __shared__ float4 tile_q[FF_DIRECT_PAIRS * 3];
     const int t = threadIdx.x;
@@ -65,7 +81,8 @@ ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n,
                     float2 rinv = ff_rsqrt2(r2);
                     if (2 * (c0 + i) == t) rinv.x = 0.0f;          // j != k (Alg. 1 line 5): r2 = 0 gave NaN, dropped here
                     if (2 * (c0 + i) + 1 == t) rinv.y = 0.0f;
-                    ff_pair2_accum(q1, q2, tg, dx, dy, dz, rinv, s);
+                    if (LJ) ff_pair2_accum<true>(q1, q2, tg, dx, dy, dz, rinv, s, ff_lj2(r2, rinv, lj));
+                    else ff_pair2_accum(q1, q2, tg, dx, dy, dz, rinv, s);
                 }
             } else {
 #pragma unroll 4
@@ -73,7 +90,9 @@ ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n,
                     const float4 q0 = q[3 * i], q1 = q[3 * i + 1], q2 = q[3 * i + 2];
                     float2 dx, dy, dz, r2;
                     ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
-                    ff_pair2_accum(q1, q2, tg, dx, dy, dz, ff_rsqrt2(r2), s);
+                    const float2 rinv = ff_rsqrt2(r2);
+                    if (LJ) ff_pair2_accum<true>(q1, q2, tg, dx, dy, dz, rinv, s, ff_lj2(r2, rinv, lj));
+                    else ff_pair2_accum(q1, q2, tg, dx, dy, dz, rinv, s);
                 }
             }
             acc[0] += s.hx.x + s.hx.y; acc[1] += s.hy.x + s.hy.y; acc[2] += s.hz.x + s.hz.y;
@@ -108,7 +127,8 @@ ff_k_direct_reduce(const double* __restrict__ part, int n, int splits, float* __
     if (F_out) { F_out[3 * (size_t)k] = (float)acc[3]; F_out[3 * (size_t)k + 1] = (float)acc[4]; F_out[3 * (size_t)k + 2] = (float)acc[5]; }
 }
 
-int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n64, float* H_out, float* F_out)
+int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n64, float* H_out, float* F_out,
+                     float lj_eps, float lj_sigma, float lj_cutoff)
 {
     int n = (int)n64;
     int tblocks = (n + FF_DIRECT_THREADS - 1) / FF_DIRECT_THREADS;
@@ -119,7 +139,11 @@ int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n64,
     while (splits > 1 && (int64_t)splits * n > FF_DIRECT_SPLIT_ELEMS) --splits;
     if (splits < 1) splits = 1;
     dim3 grid(tblocks, splits);
-    FF_LAUNCH(c, ff_k_direct, grid, FF_DIRECT_THREADS, 0, pos, mom, n, splits, c->direct_part, H_out, F_out);
+    ff_lj lj = { 24.0f * lj_eps, lj_sigma * lj_sigma, lj_cutoff * lj_cutoff };
+    if (lj_eps != 0.0f)
+        FF_LAUNCH(c, ff_k_direct<true>, grid, FF_DIRECT_THREADS, 0, pos, mom, n, splits, c->direct_part, H_out, F_out, lj);
+    else
+        FF_LAUNCH(c, ff_k_direct<false>, grid, FF_DIRECT_THREADS, 0, pos, mom, n, splits, c->direct_part, H_out, F_out, lj);
     if (splits > 1)
         FF_LAUNCH(c, ff_k_direct_reduce, (n + 255) / 256, 256, 0, c->direct_part, n, splits, H_out, F_out);
     return FF_OK;

@@ -46,8 +46,12 @@ __device__ __forceinline__ void ff_pair2_geom(const float4& q0, const float4& q1
     r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
 }
 
+// EXTRA: `extra` is added to the coefficient of rho in f (the all-pairs MD step puts the Lennard-Jones term of
+// Eq. 13 there: f^sr_kj = w rho with w = 24 eps [ (s/r)^12 - (s/r)^6 ] / r^2, PAPER.md:74 and Algorithm 1 line 8)
+template <bool EXTRA = false>
 __device__ __forceinline__ void ff_pair2_accum(const float4& q1, const float4& q2, const ff_target2& t, float2 dx,
-                                               float2 dy, float2 dz, float2 rinv, ff_acc2& s)
+                                               float2 dy, float2 dz, float2 rinv, ff_acc2& s,
+                                               float2 extra = make_float2(0.f, 0.f))
 {
     const float2 mx = make_float2(q1.z, q1.w), my = make_float2(q2.x, q2.y), mz = make_float2(q2.z, q2.w);
     const float2 rinv2 = __fmul2_rn(rinv, rinv);
@@ -61,7 +65,8 @@ __device__ __forceinline__ void ff_pair2_accum(const float4& q1, const float4& q
     s.hx = __ffma2_rn(ca, dx, s.hx); s.hy = __ffma2_rn(ca, dy, s.hy); s.hz = __ffma2_rn(ca, dz, s.hz);
     s.hx = __ffma2_rn(nr3, mx, s.hx); s.hy = __ffma2_rn(nr3, my, s.hy); s.hz = __ffma2_rn(nr3, mz, s.hz);
     const float2 w = __fmul2_rn(__fmul2_rn(ca, b), rinv2);                         // 3 (u_j.rho)(u_k.rho) / r^7
-    const float2 cr = __ffma2_rn(ff_dup(-5.0f), w, __fmul2_rn(c, r5));
+    float2 cr = __ffma2_rn(ff_dup(-5.0f), w, __fmul2_rn(c, r5));
+    if (EXTRA) cr = __fadd2_rn(cr, extra);
     s.fx = __ffma2_rn(cr, dx, s.fx); s.fy = __ffma2_rn(cr, dy, s.fy); s.fz = __ffma2_rn(cr, dz, s.fz);
     s.fx = __ffma2_rn(cb, mx, s.fx); s.fy = __ffma2_rn(cb, my, s.fy); s.fz = __ffma2_rn(cb, mz, s.fz);
     s.sk = __fadd2_rn(s.sk, ca);

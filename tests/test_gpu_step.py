@@ -47,12 +47,16 @@ def _params(ff, **kw):
         p.wall_hi[a] = kw.get("wall_hi", (0.0, 0.0, 0.0))[a]
     p.wall_epsilon = kw.get("wall_eps", 0.0)
     p.wall_sigma = kw.get("wall_sigma", 0.5)
+    p.all_pairs = 1 if kw.get("all_pairs", False) else 0
     return p
 
 
 def _oracle_step(x, v, u, w, theta, kw):
     """fp64 step from the fp32 state (x, v, u, w) the GPU started from."""
-    H, F, _, _, Q = oracle.barnes_hut(x, u, theta, 32, scale=True)
+    if kw.get("all_pairs", False):
+        H, F, Q = oracle.allpairs(x, u, scale=True)
+    else:
+        H, F, _, _, Q = oracle.barnes_hut(x, u, theta, 32, scale=True)
     fsr = lj_force(x, kw["eps"], kw["sigma"], kw["cutoff"]) if kw.get("eps", 0.0) != 0.0 else None
     if kw.get("wall_eps", 0.0) != 0.0:
         fw = wall_force(x, kw["wall_lo"], kw["wall_hi"], kw["wall_eps"], kw["wall_sigma"], kw.get("cutoff", 2.5))
@@ -202,3 +206,22 @@ def test_monolayer_between_walls(ff):
     # same interaction sets as the oracle on the flat tree
     cnt = oracle.barnes_hut(x, u, 0.5, 32)[2]
     assert ctx.counters() == cnt
+
+
+@pytest.mark.parametrize("N", [1000, 3001])
+def test_all_pairs_step_matches_oracle(ff, N):
+    """The paper's All-Pairs step (Algorithm 1): h^dip, f^dip and f^sr from one exact pair loop,
+    no tree; against the oracle's all-pairs sums + Eq. 13 + the same update."""
+    kw = dict(KW, all_pairs=True, wall_lo=(-5.0, -5.0, -5.0), wall_hi=(60.0, 60.0, 60.0), wall_eps=0.3, wall_sigma=0.5)
+    x, v, u, w = _state(1, N, 4)
+    ctx = ff.FFContext(N, 0.5)
+    dx, dv, du, dw = _dev(x), _dev(v), _dev(u), _dev(w)
+    ctx.step(dx, dv, du, dw, _params(ff, **kw), 0)
+    after = [t.cpu().numpy() for t in (dx, dv, du, dw)]
+    ref, aux = _oracle_step(x, v, u, w, 0.5, kw)
+    _check_step((x, v, u, w), after, ref, aux, kw)
+    # and the Barnes-Hut step from the same state differs from it only by the approximation error of the tree
+    dx2, dv2, du2, dw2 = _dev(x), _dev(v), _dev(u), _dev(w)
+    ctx.step(dx2, dv2, du2, dw2, _params(ff, **dict(kw, all_pairs=False)), 0)
+    dvel = (dv2 - dv).double().norm() / (dv - _dev(v)).double().norm()
+    assert 0.0 < float(dvel) < 0.05
