@@ -82,3 +82,32 @@ def test_average_dipole_field_barnes_hut_vs_all_pairs():
     # the per-particle fields differ by the percent-level error of Eq. 14's lowest-order cell
     rel = float((Hb - Hd).double().norm() / Hd.double().norm())
     assert rel < 0.06
+
+
+def test_magnetisation_all_pairs_and_barnes_hut_agree():
+    """PAPER.md:233, Fig. 3(b): the magnetisation of N = 10^3 particles from the All-Pairs and the Barnes-Hut
+    algorithm, "almost identical".  Same initial state and noise stream for both; each must follow L(alpha)."""
+    import torch
+    import paper_1212_2934_b200 as ff
+    N, T, G, alpha = 1024, 4.0, 2.0, 2.0
+    pos, mom, L = ffgen.ensemble(N, 0.01, "isotropic", 5.0, 31)
+    res = {}
+    for name, flag in (("bh", 0), ("ap", 1)):
+        p = ff.ff_step_params()
+        p.dtau, p.gamma_d, p.gamma_r = 2e-3, G, G
+        p.h_ext[2] = alpha * T
+        p.lj_epsilon, p.lj_sigma, p.lj_cutoff = 1.0, 1.0, 2.5
+        p.noise_r, p.noise_d, p.seed = 2.5 * np.sqrt(2 * G * T), np.sqrt(2 * G * T), 3
+        p.all_pairs = flag
+        x, u = torch.from_numpy(pos).cuda(), torch.from_numpy(mom).cuda()
+        v, w = torch.zeros_like(x), torch.zeros_like(x)
+        ctx = ff.FFContext(N, 0.5)
+        uz = []
+        for s in range(6000):
+            ctx.step(x, v, u, w, p, s)
+            if s >= 1000 and s % 20 == 0:
+                uz.append(float(u[:, 2].double().mean()))
+        res[name] = float(np.mean(uz))
+    lang = _langevin(alpha)
+    assert abs(res["ap"] - lang) <= 0.04 * lang and abs(res["bh"] - lang) <= 0.04 * lang, (res, lang)
+    assert abs(res["ap"] - res["bh"]) <= 0.03 * lang, res
