@@ -436,8 +436,27 @@ def run_ours(args):
                        "noise": [0.05, 0.05]},
             "note": "L2 not flushed between these steps (back-to-back MD steps, as in a simulation)"}
 
-    # ---- the oracle timed beside it on this box's host cores (bounded sample)
+    # ---- parity of this very run at full size: the oracle's Barnes-Hut on sampled groups (DESIGN.md section 6 metric)
     import oracle
+    otree = oracle.Tree(c["pos"])
+    otree.moments(c["mom"])
+    sel = np.random.default_rng(7).choice((N + 31) // 32, min(256, (N + 31) // 32), replace=False)
+    Ho, Fo, _, Qo = otree.eval(theta, 32, groups=sel, scale=True)
+    _, operm = otree.keys()
+    rows = operm[(sel[:, None] * 32 + np.arange(32)[None, :]).ravel().clip(max=N - 1)]
+    rows = np.unique(rows)
+    Hg, Fg = H.cpu().numpy().astype(np.float64), F.cpu().numpy().astype(np.float64)
+
+    def _errs(x, ref, q):
+        e = np.linalg.norm(x - ref, axis=1) / np.maximum(np.linalg.norm(ref, axis=1), q / 8.0)
+        return {"max": float(e.max()), "p99": float(np.quantile(e, 0.99)), "median": float(np.median(e)),
+                "global_rel_l2": float(np.linalg.norm(x - ref) / np.linalg.norm(ref))}
+    parity = {"targets": int(len(rows)), "tolerance": 1e-4,
+              "H": _errs(Hg[rows], Ho[rows], Qo[rows, 0]), "F": _errs(Fg[rows], Fo[rows], Qo[rows, 1]),
+              "metric": "|x_k - ref_k| / max(|ref_k|, Q_k / 8) against the fp64 oracle's Barnes-Hut (same theta, W = 32)"}
+    del otree
+
+    # ---- the oracle timed beside it on this box's host cores (bounded sample)
     cores = oracle.max_threads()
     sample = 2048 if N >= (1 << 20) else max(1, min(2048, (N + 31) // 32))
     cpu_value, cpu_detail = _oracle_rate(c, sample)
@@ -459,7 +478,7 @@ def run_ours(args):
                 "steps": e2e_steps, "api": "ff_eval_bh_host_async + ff_host_sync (pinned host buffers, steps pipelined over three "
                                            "streams; the 512 MB L2 flush of every step is inside the timed region)",
                 "one_step_at_a_time_ms": e2e_serial_ms, "checksum": checksum},
-        "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "roofline": roofline, "cpu_baseline": cpu_baseline, "parity_at_full_size": parity,
         "phases_ms": phases, "hbm_phases": hbm_phases,
         "counters": {"n_cell": n_cell, "n_particle": n_part, "n_mac_tests": n_mac,
                      "interactions_per_target": interactions / N},
