@@ -275,7 +275,7 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for i in range(e2e_steps):
-        flush.zero_()                                  # evict the previous step from L2 (inside the timed region here)
+        flush[:192 << 20].zero_()                      # evict the previous step from the 126 MB L2 (inside the timed region here)
         ctx.eval_bh_host_async(pos_h, mom_h, H_h[i & 1], F_h[i & 1])
     ctx.host_sync()
     e1.record()
@@ -476,7 +476,7 @@ def run_ours(args):
         "clocks": clocks, "gpu_launches": int(launches), "launches_per_step": launches / args.steps,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 12, "d2h_bytes_per_step": 2 * N * 12,
                 "steps": e2e_steps, "api": "ff_eval_bh_host_async + ff_host_sync (pinned host buffers, steps pipelined over three "
-                                           "streams; the 512 MB L2 flush of every step is inside the timed region)",
+                                           "streams; a 192 MB L2 flush before every step is inside the timed region)",
                 "one_step_at_a_time_ms": e2e_serial_ms, "checksum": checksum},
         "roofline": roofline, "cpu_baseline": cpu_baseline, "parity_at_full_size": parity,
         "phases_ms": phases, "hbm_phases": hbm_phases,
