@@ -121,6 +121,18 @@ def max_over_ranks(ms, world, device):
     return float(t.item())
 
 
+def gather_particles(local, world):
+    """Target sharding: every rank owns N / world particles and needs all of them as sources.
+    One all-gather per array and step (12 B per particle and array); the tree is then built redundantly."""
+    if world == 1:
+        return local
+    import torch
+    import torch.distributed as dist
+    parts = [torch.empty_like(local) for _ in range(world)]
+    dist.all_gather(parts, local.contiguous())
+    return torch.cat(parts, dim=0)
+
+
 def job_rate(world, units_per_rank, ms):
     """Whole-job throughput: every rank processed `units_per_rank` units (weak scaling, independent replicas,
     no data-path collective) in `ms`, the max over ranks."""
@@ -203,7 +215,9 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    c = _workload(args.n, rank, args.config)          # independent replica per rank
+    sharded = args.shard == "targets" and world > 1
+    # replicas: an independent realisation per rank; target sharding: ONE ensemble, every rank owns N / world rows
+    c = _workload(args.n, 0 if sharded else rank, args.config)
     N, theta = c["N"], c["theta"]
     pos_h = torch.from_numpy(c["pos"]).pin_memory()
     mom_h = torch.from_numpy(c["mom"]).pin_memory()
@@ -212,9 +226,20 @@ def run_ours(args):
     ctx = ff.FFContext(N, theta, device=dev, timing=True)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
+    if sharded:
+        assert N % world == 0, "target sharding needs N divisible by the number of ranks"
+        rows = slice(rank * (N // world), (rank + 1) * (N // world))
+        pos_local, mom_local = pos[rows].clone(), mom[rows].clone()
+        g_begin, g_end = ff.shard_groups(N, world, rank)
+
     def step():
-        ctx.build_tree(pos)
-        ctx.eval_bh(pos, mom, H, F)
+        if sharded:
+            p_all, m_all = gather_particles(pos_local, world), gather_particles(mom_local, world)
+            ctx.build_tree(p_all)
+            ctx.eval_bh_range(p_all, m_all, H, F, g_begin, g_end)
+        else:
+            ctx.build_tree(pos)
+            ctx.eval_bh(pos, mom, H, F)
 
     # interaction counts of this workload (separate, untimed run of the counting kernel variant)
     ctx.set_option(ff.FF_OPT_COUNTERS, 1)
@@ -257,7 +282,7 @@ def run_ours(args):
     total_ms = max_over_ranks(sum(step_ms), world, dev)
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     ms_per_step = total_ms / args.steps
-    value = job_rate(world, N, ms_per_step)
+    value = job_rate(1 if sharded else world, N, ms_per_step)     # sharded: the ranks share ONE ensemble of N
     phases = {k: v / args.steps for k, v in phases.items()}
 
     # ---- end to end through the C ABI with host buffers (H2D + step + D2H of every step inside the timed region).
@@ -288,7 +313,8 @@ def run_ours(args):
         ctx.eval_bh_host(pos_h, mom_h, H_h[0], F_h[0])
     e2e_serial_ms = (time.perf_counter() - t0) * 1e3 / 3
     H_h, F_h = H_h[0], F_h[0]
-    e2e_value = job_rate(world, N, max_over_ranks(e2e_ms, world, dev) / e2e_steps)
+    # (with --shard targets this stays the single-GPU host call of every rank: reported per GPU, not summed)
+    e2e_value = job_rate(1 if sharded else world, N, max_over_ranks(e2e_ms, world, dev) / e2e_steps)
     checksum = float(H_h.double().abs().sum() + F_h.double().abs().sum())
 
     if rank != 0:
@@ -325,7 +351,7 @@ def run_ours(args):
                   for k in alg_bytes if phases[k] > 0}
 
     extras = {}
-    if not args.quick and N <= (1 << 21):                  # the N^2 kernel takes minutes beyond that
+    if not args.quick and not sharded and N <= (1 << 21):                  # the N^2 kernel takes minutes beyond that
         # GPU direct all-pairs on the same workload (a8), once; and the BH-vs-all-pairs error vs theta
         torch.cuda.synchronize()
         ctx.timings()
@@ -440,7 +466,8 @@ def run_ours(args):
     import oracle
     otree = oracle.Tree(c["pos"])
     otree.moments(c["mom"])
-    sel = np.random.default_rng(7).choice((N + 31) // 32, min(256, (N + 31) // 32), replace=False)
+    g_lo, g_hi = (g_begin, g_end) if sharded else (0, (N + 31) // 32)
+    sel = g_lo + np.random.default_rng(7).choice(g_hi - g_lo, min(256, g_hi - g_lo), replace=False)
     Ho, Fo, _, Qo = otree.eval(theta, 32, groups=sel, scale=True)
     _, operm = otree.keys()
     rows = operm[(sel[:, None] * 32 + np.arange(32)[None, :]).ravel().clip(max=N - 1)]
@@ -468,11 +495,14 @@ def run_ours(args):
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if sharded else "weak",
+        "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": _describe(c) + ", tree rebuilt every step, H and F",
                    "N": N, "theta": theta, "group": 32, "nleaf": 1, "l2": "flushed between timed steps (512 MB memset)",
-                   "replicas": world},
+                   "replicas": 1 if sharded else world,
+                   "sharding": "targets: one ensemble, all-gather of pos and mom per step, redundant tree, each rank walks "
+                               "a Morton-contiguous slice of the groups" if sharded else "independent replicas, no collective"},
         "clocks": clocks, "gpu_launches": int(launches), "launches_per_step": launches / args.steps,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 12, "d2h_bytes_per_step": 2 * N * 12,
                 "steps": e2e_steps, "api": "ff_eval_bh_host_async + ff_host_sync (pinned host buffers, steps pipelined over three "
@@ -500,6 +530,9 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json config whose recipe is used (default 3, the one the metric is quoted on)")
     ap.add_argument("--quick", action="store_true", help="skip the direct kernel and the theta sweep")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "targets"],
+                    help="N > 1: independent replicas per rank (default, weak scaling) or one ensemble with the "
+                         "targets sharded over the ranks (all-gather of pos and mom per step, strong scaling)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -129,6 +129,16 @@ int ff_build_tree(ff_ctx* ctx, const float* pos, int64_t n);
 int ff_eval_bh(ff_ctx* ctx, const float* pos, const float* mom, float* H_out, float* F_out);
 
 /*
+ * The same for a slice of the targets: only the walk groups [group_begin, group_end) of the SORTED order are
+ * evaluated (group g = sorted slots 32 g .. 32 g + 31; group_end < 0 means "to the last group"), and only the
+ * rows of H_out / F_out that belong to those targets (caller order, scattered) are written.  The cell moments are
+ * computed for the whole tree.  This is the unit of the target sharding of SURVEY.md 8(e): every GPU holds all
+ * sources and the whole tree and evaluates a Morton-contiguous slice of the targets; no halo, no reduction.
+ */
+int ff_eval_bh_range(ff_ctx* ctx, const float* pos, const float* mom, float* H_out, float* F_out,
+                     int64_t group_begin, int64_t group_end);
+
+/*
  * a8: exact all-pairs sum (Algorithm 1), self excluded by
  * index (line 5).  Needs no tree.  Arguments as ff_eval_bh, n given.
  */

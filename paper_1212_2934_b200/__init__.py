@@ -31,7 +31,7 @@ FF_CHILD_LEAF1, FF_CHILD_MULTI, FF_CHILD_SLOT = 0x80000000, 0x40000000, 0x3FFFFF
 # every symbol include/ff.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
     "ff_workspace_bytes", "ff_create", "ff_destroy", "ff_set_stream", "ff_set_option", "ff_build_tree",
-    "ff_eval_bh", "ff_eval_direct", "ff_eval_bh_host", "ff_eval_direct_host", "ff_step", "ff_get_tree",
+    "ff_eval_bh", "ff_eval_bh_range", "ff_eval_direct", "ff_eval_bh_host", "ff_eval_direct_host", "ff_step", "ff_get_tree",
     "ff_get_timings", "ff_eval_bh_host_async", "ff_host_sync", "ff_get_counters", "ff_get_prefilter_count", "ff_get_launch_count", "ff_measure_fp32_peak", "ff_error_string",
     "ff_last_error",
 )
@@ -53,6 +53,15 @@ class ff_tree_view(ctypes.Structure):
                 ("mom_sorted", ctypes.c_void_p), ("cell_first", ctypes.c_void_p), ("cell_end", ctypes.c_void_p),
                 ("cell_level", ctypes.c_void_p), ("child", ctypes.c_void_p), ("leaf_count", ctypes.c_void_p),
                 ("cell_centre", ctypes.c_void_p), ("cell_moment", ctypes.c_void_p)]
+
+
+def shard_groups(n: int, world: int, rank: int):
+    """Target sharding of SURVEY.md 8(e): the walk groups (32 consecutive sorted targets) of an n-particle ensemble
+    split into `world` Morton-contiguous slices of equal size (+-1); returns (group_begin, group_end) of `rank`."""
+    groups = (n + 31) // 32
+    base, rem = divmod(groups, world)
+    begin = rank * base + min(rank, rem)
+    return begin, begin + base + (1 if rank < rem else 0)
 
 
 class FFError(RuntimeError):
@@ -86,6 +95,8 @@ def lib():
         L.ff_eval_bh.argtypes = [vp, vp, vp, vp, vp]
         L.ff_eval_direct.restype = i32
         L.ff_eval_direct.argtypes = [vp, vp, vp, i64, vp, vp]
+        L.ff_eval_bh_range.restype = i32
+        L.ff_eval_bh_range.argtypes = [vp, vp, vp, vp, vp, i64, i64]
         L.ff_eval_bh_host.restype = i32
         L.ff_eval_bh_host.argtypes = [vp, vp, vp, i64, vp, vp]
         L.ff_eval_bh_host_async.restype = i32
@@ -204,6 +215,16 @@ class FFContext:
         hp = _dev_f32(H, n, "H") if H is not None else None
         fp = _dev_f32(F, n, "F") if F is not None else None
         self._check(self._L.ff_eval_bh(self._h, p, m, hp, fp), "ff_eval_bh")
+        return H, F
+
+    def eval_bh_range(self, pos, mom, H, F, group_begin: int, group_end: int = -1):
+        """ff_eval_bh_range: only the walk groups [group_begin, group_end) of the sorted order; only their rows of
+        H and F (caller order) are written."""
+        n = self.n
+        self._check(self._L.ff_eval_bh_range(self._h, _dev_f32(pos, n, "pos"), _dev_f32(mom, n, "mom"),
+                                             _dev_f32(H, n, "H") if H is not None else None,
+                                             _dev_f32(F, n, "F") if F is not None else None,
+                                             int(group_begin), int(group_end)), "ff_eval_bh_range")
         return H, F
 
     def eval_direct(self, pos, mom, H=None, F=None):

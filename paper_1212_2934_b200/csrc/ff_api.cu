@@ -158,15 +158,24 @@ extern "C" int ff_build_tree(ff_ctx* c, const float* pos, int64_t n)
 
 extern "C" int ff_eval_bh(ff_ctx* c, const float* pos, const float* mom, float* H_out, float* F_out)
 {
+    return ff_eval_bh_range(c, pos, mom, H_out, F_out, 0, -1);
+}
+
+extern "C" int ff_eval_bh_range(ff_ctx* c, const float* pos, const float* mom, float* H_out, float* F_out,
+                                int64_t group_begin, int64_t group_end)
+{
     if (!c || !pos || !mom) return FF_ERR_INVALID_ARG;
     if (!c->tree_built) return FF_ERR_NO_TREE;
+    const int64_t groups = (c->n + 31) / 32;
+    if (group_end < 0) group_end = groups;
+    if (group_begin < 0 || group_begin > group_end || group_end > groups) return FF_ERR_INVALID_ARG;
     int rc;
     ff_phase_begin(c, FF_PH_MOMENTS);
     if ((rc = ff_launch_moments(c, mom)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_MOMENTS);
     c->moments_valid = 1;
     ff_phase_begin(c, FF_PH_WALK);
-    if ((rc = ff_launch_walk(c, H_out, F_out)) != FF_OK) return rc;
+    if ((rc = ff_launch_walk(c, H_out, F_out, (int)group_begin, (int)group_end)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_WALK);
     return FF_OK;
 }

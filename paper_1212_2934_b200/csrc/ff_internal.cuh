@@ -144,7 +144,7 @@ int ff_launch_bbox_keys(ff_ctx* c, const float* pos);
 int ff_launch_sort(ff_ctx* c, const float* pos);
 int ff_launch_build(ff_ctx* c);
 int ff_launch_moments(ff_ctx* c, const float* mom);
-int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out);
+int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out, int group_begin = 0, int group_end = -1);
 int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n, float* H_out, float* F_out,
                      float lj_eps = 0.0f, float lj_sigma = 1.0f, float lj_cutoff = 0.0f);   // lj_eps != 0: F_out = f^dip + f^sr
 int ff_launch_fp32_peak(ff_ctx* c, int iters, double* tflops);

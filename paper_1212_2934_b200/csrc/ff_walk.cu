@@ -356,7 +356,7 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
 // and consecutive (spatially adjacent) groups run at the same time and share cells in L1/L2.
 template <bool COUNT>
 __global__ void __launch_bounds__(FF_WALK_WARPS * 32, FF_WALK_MINB)
-ff_k_walk(int n, float theta, ff_globals* __restrict__ g, const float4* __restrict__ pos_s,
+ff_k_walk(int n, int group_begin, int group_end, float theta, ff_globals* __restrict__ g, const float4* __restrict__ pos_s,
           const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
           const int32_t* __restrict__ cell_first,
           const int32_t* __restrict__ cell_end, const int4* __restrict__ cell_child,
@@ -367,11 +367,11 @@ ff_k_walk(int n, float theta, ff_globals* __restrict__ g, const float4* __restri
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     ff_walk_smem& sm = reinterpret_cast<ff_walk_smem*>(smem_raw)[w];
-    const int groups = (n + 31) >> 5;
+    const int groups = group_end;                          // groups [group_begin, group_end) of the sorted order
     const int n_cells = g->n_cells;
     for (;;) {
         int grp = 0;
-        if (lane == 0) grp = atomicAdd(&g->walk_next, 1);
+        if (lane == 0) grp = group_begin + atomicAdd(&g->walk_next, 1);
         grp = __shfl_sync(FF_FULL, grp, 0);
         if (grp >= groups) break;
         ff_walk_group<COUNT>(sm, grp, lane, n, theta, n_cells, pos_s, mom_s, perm, cell_first, cell_end, cell_child,
@@ -380,10 +380,12 @@ ff_k_walk(int n, float theta, ff_globals* __restrict__ g, const float4* __restri
     }
 }
 
-int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out)
+int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out, int group_begin, int group_end)
 {
     int n = (int)c->n;
-    int groups = (n + 31) / 32;
+    if (group_end < 0) group_end = (n + 31) / 32;
+    int groups = group_end - group_begin;
+    if (groups <= 0) return FF_OK;
     size_t smem = sizeof(ff_walk_smem) * FF_WALK_WARPS;
     int* per_sm = c->occ_walk;                             // per context: contexts may live on different devices
     if (!per_sm[0]) {
@@ -397,11 +399,11 @@ int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out)
     int blocks = min(c->num_sms * per_sm[cnt], (groups + FF_WALK_WARPS - 1) / FF_WALK_WARPS);
     if (cnt) {
         FF_CUDA(c, cudaMemsetAsync(c->g->counters, 0, sizeof(c->g->counters), c->stream));
-        FF_LAUNCH(c, ff_k_walk<true>, blocks, FF_WALK_WARPS * 32, smem, n, c->theta, c->g, c->pos_s, c->mom_s,
+        FF_LAUNCH(c, ff_k_walk<true>, blocks, FF_WALK_WARPS * 32, smem, n, group_begin, group_end, c->theta, c->g, c->pos_s, c->mom_s,
                   c->idx[0], c->cell_first, c->cell_end, (const int4*)c->cell_child,
                   c->leaf_count, c->cell_centre, c->cell_moment, H_out, F_out, c->g->counters);
     } else {
-        FF_LAUNCH(c, ff_k_walk<false>, blocks, FF_WALK_WARPS * 32, smem, n, c->theta, c->g, c->pos_s, c->mom_s,
+        FF_LAUNCH(c, ff_k_walk<false>, blocks, FF_WALK_WARPS * 32, smem, n, group_begin, group_end, c->theta, c->g, c->pos_s, c->mom_s,
                   c->idx[0], c->cell_first, c->cell_end, (const int4*)c->cell_child,
                   c->leaf_count, c->cell_centre, c->cell_moment, H_out, F_out, c->g->counters);
     }

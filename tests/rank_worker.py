@@ -25,8 +25,17 @@ def main():
     dist.barrier()
     ms = bench.max_over_ranks(fake_ms, world, torch.device("cpu"))
     rate = bench.job_rate(world, c["N"], ms)
+    # target sharding: one common ensemble, every rank owns N / world rows and gathers the rest
+    import paper_1212_2934_b200 as ff            # import only: no library call, no GPU
+    common = bench._workload(2048, 0, 3)
+    full = torch.from_numpy(common["pos"])
+    n_loc = common["N"] // world
+    mine = full[rank * n_loc:(rank + 1) * n_loc].clone()
+    gathered = bench.gather_particles(mine, world)
+    gb, ge = ff.shard_groups(common["N"], world, rank)
     rec = {"rank": rank, "world": world, "local": local, "ms": ms, "rate": rate, "N": c["N"],
-           "pos_sum": float(np.asarray(c["pos"], np.float64).sum())}
+           "pos_sum": float(np.asarray(c["pos"], np.float64).sum()),
+           "gather_ok": bool(torch.equal(gathered, full)), "groups": [gb, ge]}
     with open(os.path.join(out_dir, "rank%d.json" % rank), "w") as fh:
         json.dump(rec, fh)
     if rank == 0:

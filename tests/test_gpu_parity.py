@@ -273,6 +273,36 @@ def test_pipelined_host_calls(ff):
     assert np.array_equal(H.cpu().numpy(), ref[0][0])
 
 
+def test_target_ranges_compose_to_the_full_evaluation(ff, cfg1):
+    """ff_eval_bh_range (the unit of target sharding): slices written by separate calls into the
+    same arrays reproduce the full evaluation bit for bit; rows outside a slice are left untouched."""
+    import torch
+    pos, mom = _dev(cfg1["pos"]), _dev(cfg1["mom"])
+    N = len(cfg1["pos"])
+    ctx = ff.FFContext(N, 0.5)
+    ctx.build_tree(pos)
+    H0, F0 = ctx.eval_bh(pos, mom)
+    H = torch.full_like(H0, float("nan"))
+    F = torch.full_like(F0, float("nan"))
+    world = 3
+    slices = [ff.shard_groups(N, world, r) for r in range(world)]
+    assert slices[0][0] == 0 and slices[-1][1] == (N + 31) // 32
+    assert all(a[1] == b[0] for a, b in zip(slices, slices[1:]))
+    ctx.eval_bh_range(pos, mom, H, F, *slices[1])
+    torch.cuda.synchronize()
+    perm = ctx.get_tree()["perm"].astype(np.int64)
+    mine = np.zeros(N, bool)
+    mine[perm[slices[1][0] * 32: min(N, slices[1][1] * 32)]] = True
+    Hn = H.cpu().numpy()
+    assert np.isnan(Hn[~mine]).all() and np.array_equal(Hn[mine], H0.cpu().numpy()[mine])
+    ctx.eval_bh_range(pos, mom, H, F, *slices[0])
+    ctx.eval_bh_range(pos, mom, H, F, *slices[2])
+    torch.cuda.synchronize()
+    assert torch.equal(H, H0) and torch.equal(F, F0)
+    with pytest.raises(ff.FFError):
+        ctx.eval_bh_range(pos, mom, H, F, 5, 3)
+
+
 def test_error_codes(ff):
     ctx = ff.FFContext(100, 0.5)
     p = _dev(ffgen.uniform_points(100, 5.0, 0))

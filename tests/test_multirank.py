@@ -32,6 +32,9 @@ def test_two_rank_replicas_max_time_and_job_rate(tmp_path):
     assert all(abs(x["rate"] - 2 * 2048 / 20e-3) < 1e-6 for x in recs)
     # independent replicas: same recipe and size, different seed
     assert recs[0]["N"] == recs[1]["N"] == 2048 and recs[0]["pos_sum"] != recs[1]["pos_sum"]
+    # target sharding: the all-gather re-assembles the common ensemble on every rank, the group slices tile it
+    assert all(x["gather_ok"] for x in recs)
+    assert recs[0]["groups"] == [0, 32] and recs[1]["groups"] == [32, 64]
     # exactly one JSON line, from rank 0
     lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1 and json.loads(lines[0])["n_gpus"] == 2
