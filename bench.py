@@ -339,6 +339,10 @@ def run_ours(args):
         "interactions_per_launch": interactions, "flop_per_interaction": FLOP_PER_INTERACTION,
         "kernel_ms": walk_ms, "kernel_share_of_step": walk_ms / ms_per_step,
         "interactions_per_s": interactions / (walk_ms * 1e-3),
+        # FP32-pipe occupancy by the interaction arithmetic alone = interactions x 38 FP32 lane-ops
+        # (19 packed instructions of two lanes' worth each) / (time x SMs x 128 lanes x clock)
+        "fp32_lane_ops_per_interaction": 38,
+        "fp32_lane_occupancy_by_interactions": interactions * 38.0 / (walk_ms * 1e-3 * num_sms * FP32_LANES_PER_SM * sm_max * 1e6),
         "note": "21 of the 38 FP32 instructions per interaction are FMAs, so a saturated FP32 pipe reads 0.78; packed "
                 "FFMA2 with three register-pair operands issues every 3 cycles (profiles/r1_walk_full.md), which caps "
                 "this instruction mix near 0.60",
