@@ -124,6 +124,74 @@ def canonical_from_oracle(tree):
             zip(nd["first"], nd["level"], nd["prefix"], nd["count"], nd["is_leaf"])]
 
 
+# ---- an independently written list builder (python, exact fp32 emulation) ---
+def build_lists(pos, mom, theta, W, nleaf):
+    """Per group: (accepted cells as (level, prefix), leaf particles as sorted slots), using only
+    brute-force prefix grouping and the plain statement of the rule."""
+    nodes, sk, perm, lo, S = brute_tree(pos, nleaf)
+    sp = np.asarray(pos, np.float32)[perm]
+    sm = np.asarray(mom, np.float32)[perm]
+    N = len(sp)
+    info = {}
+    for (f, l, p, c, leaf) in nodes:
+        cen = (np.sum(sp[f:f + c].astype(np.float64), axis=0) / c).astype(np.float32)
+        mu = np.sum(sm[f:f + c].astype(np.float64), axis=0).astype(np.float32)
+        info[(l, p)] = (f, c, leaf, cen, mu)
+    th2 = np.float32(np.float32(theta) * np.float32(theta))
+    out = []
+    for g0 in range(0, N, W):
+        g1 = min(N, g0 + W)
+        cells, parts = [], []
+        stack = [(0, 0)]
+        while stack:
+            l, p = stack.pop()
+            f, c, leaf, cen, mu = info[(l, p)]
+            if leaf:
+                parts.extend(range(f, f + c))
+                continue
+            holds_member = f < g1 and f + c > g0
+            if not holds_member:
+                s = np.float32(S) * np.float32(2.0 ** -l)
+                s2 = np.float32(s * s)
+                if all(member_accepts(sp[k], cen, s2, th2) for k in range(g0, g1)):
+                    cells.append((l, p))
+                    continue
+            for o in range(7, -1, -1):
+                if (l + 1, p << 3 | o) in info:
+                    stack.append((l + 1, p << 3 | o))
+        out.append((g0, g1, cells, parts))
+    return out, info, sp, sm, perm
+
+
+def eval_lists(lists, info, sp, sm, perm, scale=False):
+    N = len(sp)
+    H = np.zeros((N, 3))
+    F = np.zeros((N, 3))
+    Q = np.zeros((N, 2))
+    for g0, g1, cells, parts in lists:
+        for k in range(g0, g1):
+            h = np.zeros(3)
+            f = np.zeros(3)
+            q = np.zeros(2)
+            for key in cells:
+                _, _, _, cen, mu = info[key]
+                dh, df = pair_terms(sp[k], sm[k], cen, mu)
+                h += dh
+                f += df
+                q += (dh @ dh, df @ df)
+            for j in parts:
+                if j == k:
+                    continue
+                dh, df = pair_terms(sp[k], sm[k], sp[j], sm[j])
+                h += dh
+                f += df
+                q += (dh @ dh, df @ df)
+            H[perm[k]] = h
+            F[perm[k]] = f
+            Q[perm[k]] = np.sqrt(q)      # root-sum-square of the terms of particle k's own sum (DESIGN.md section 6)
+    return (H, F, Q) if scale else (H, F)
+
+
 # ---- error metric of DESIGN.md ("error metric", reading Q19) ------------------
 KAPPA = 8.0
 
@@ -148,8 +216,16 @@ def rel_err(x, ref, Q=None):
     return float(e.max()), float(np.median(e)), float(np.percentile(e, 99)), float(glob)
 
 
-def check_hf(H, F, Ho, Fo, Q, tol):
-    """Assert both fields within tol under the metric above; returns the two error tuples."""
+def check_hf(H, F, Ho, Fo, Q, tol, survey=True):
+    """Assert both fields within tol; returns the error tuples.
+
+    Two gates.  (1) the term-scale metric e_k = |dx_k| / max(|ref_k|, Q_k / KAPPA), always.
+    (2) survey=True: ALSO the survey's metric (floor 1e-3 rms |ref|, no Q), so that wherever the sums
+    do not cancel the result does not depend on the oracle's Q at all.  survey=False is reserved for the inputs whose
+    sums cancel by construction (head-to-tail chains: config 4 and the chain cases of the sweep), named in DESIGN.md."""
     eh, ef = rel_err(H, Ho, Q[:, 0]), rel_err(F, Fo, Q[:, 1])
-    assert eh[0] <= tol and ef[0] <= tol, (eh, ef)
+    assert eh[0] <= tol and ef[0] <= tol, ("term-scale metric", eh, ef)
+    if survey:
+        sh, sf = rel_err(H, Ho), rel_err(F, Fo)
+        assert sh[0] <= tol and sf[0] <= tol, ("survey metric (no Q)", sh, sf)
     return eh, ef

@@ -7,70 +7,7 @@ import pytest
 
 import ffgen
 import oracle
-from helpers import brute_tree, member_accepts, pair_terms, rel_err
-
-
-# ---- an independently written list builder (python, exact fp32 emulation) ---
-def _build_lists(pos, mom, theta, W, nleaf):
-    """Per group: (accepted cells as (level, prefix), leaf particles as sorted slots), using only
-    brute-force prefix grouping and the plain statement of the rule."""
-    nodes, sk, perm, lo, S = brute_tree(pos, nleaf)
-    sp = np.asarray(pos, np.float32)[perm]
-    sm = np.asarray(mom, np.float32)[perm]
-    N = len(sp)
-    info = {}
-    for (f, l, p, c, leaf) in nodes:
-        cen = (np.sum(sp[f:f + c].astype(np.float64), axis=0) / c).astype(np.float32)
-        mu = np.sum(sm[f:f + c].astype(np.float64), axis=0).astype(np.float32)
-        info[(l, p)] = (f, c, leaf, cen, mu)
-    th2 = np.float32(np.float32(theta) * np.float32(theta))
-    out = []
-    for g0 in range(0, N, W):
-        g1 = min(N, g0 + W)
-        cells, parts = [], []
-        stack = [(0, 0)]
-        while stack:
-            l, p = stack.pop()
-            f, c, leaf, cen, mu = info[(l, p)]
-            if leaf:
-                parts.extend(range(f, f + c))
-                continue
-            holds_member = f < g1 and f + c > g0
-            if not holds_member:
-                s = np.float32(S) * np.float32(2.0 ** -l)
-                s2 = np.float32(s * s)
-                if all(member_accepts(sp[k], cen, s2, th2) for k in range(g0, g1)):
-                    cells.append((l, p))
-                    continue
-            for o in range(7, -1, -1):
-                if (l + 1, p << 3 | o) in info:
-                    stack.append((l + 1, p << 3 | o))
-        out.append((g0, g1, cells, parts))
-    return out, info, sp, sm, perm
-
-
-def _eval_lists(lists, info, sp, sm, perm):
-    N = len(sp)
-    H = np.zeros((N, 3))
-    F = np.zeros((N, 3))
-    for g0, g1, cells, parts in lists:
-        for k in range(g0, g1):
-            h = np.zeros(3)
-            f = np.zeros(3)
-            for key in cells:
-                _, _, _, cen, mu = info[key]
-                dh, df = pair_terms(sp[k], sm[k], cen, mu)
-                h += dh
-                f += df
-            for j in parts:
-                if j == k:
-                    continue
-                dh, df = pair_terms(sp[k], sm[k], sp[j], sm[j])
-                h += dh
-                f += df
-            H[perm[k]] = h
-            F[perm[k]] = f
-    return H, F
+from helpers import build_lists as _build_lists, eval_lists as _eval_lists, pair_terms, rel_err
 
 
 @pytest.mark.parametrize("N,W,nleaf,theta,seed", [
