@@ -61,8 +61,8 @@ enum {
     FF_OPT_NLEAF = 2,     /* leaf capacity N_leaf >= 1; 1 = the paper's tree. Invalidates the tree. */
     FF_OPT_COUNTERS = 3,  /* != 0: the walk also counts interactions (slower); read with ff_get_counters */
     FF_OPT_TIMING = 4,    /* != 0: record CUDA events around each phase; read with ff_get_timings */
-    FF_OPT_GROUP = 5      /* targets per walk group W (reading Q2).  The GPU walk implements W = 32, one
-                             warp per group; any other value is FF_ERR_INVALID_ARG (the oracle takes any W) */
+    FF_OPT_GROUP = 5      /* targets per walk group W (reading Q2): 32 (default) or 64, one warp per group with
+                             two targets per lane; any other value is FF_ERR_INVALID_ARG (the oracle takes any W) */
 };
 
 /* phases reported by ff_get_timings, in launch order */
@@ -119,7 +119,7 @@ int ff_build_tree(ff_ctx* ctx, const float* pos, int64_t n);
  * H_out / F_out: device [n][3] fp32, either may be NULL to skip it.
  * H_out = sum_{j != k} h_kj only (no external field); F_out = f_k of Eq. 12,
  * no prefactor.  Opening rule (reading O5): targets are walked in
- * groups of 32 consecutive sorted particles (one warp); a leaf's particles
+ * groups of W = 32 (FF_OPT_GROUP: or 64) consecutive sorted particles (one warp); a leaf's particles
  * are summed directly (self skipped by index); an internal cell is opened if
  * its range holds a member of the group, else accepted for the whole group
  * iff every member k satisfies, in fp32 and exactly this order,
@@ -130,7 +130,7 @@ int ff_eval_bh(ff_ctx* ctx, const float* pos, const float* mom, float* H_out, fl
 
 /*
  * The same for a slice of the targets: only the walk groups [group_begin, group_end) of the SORTED order are
- * evaluated (group g = sorted slots 32 g .. 32 g + 31; group_end < 0 means "to the last group"), and only the
+ * evaluated (group g = sorted slots W g .. W g + W - 1; group_end < 0 means "to the last group"), and only the
  * rows of H_out / F_out that belong to those targets (caller order, scattered) are written.  The cell moments are
  * computed for the whole tree.  This is the unit of the target sharding of SURVEY.md 8(e): every GPU holds all
  * sources and the whole tree and evaluates a Morton-contiguous slice of the targets; no halo, no reduction.
@@ -210,8 +210,9 @@ int ff_step(ff_ctx* ctx, float* pos, float* vel, float* mom, float* angvel, int6
  * Introspection for tests and measurement.  Pointers are DEVICE pointers into
  * the workspace, valid until the next ff_build_tree / ff_step / ff_destroy.
  * Synchronises the stream.  Internal cells are numbered in pre-order, i.e.
- * sorted by (first, level).  child[8*i + o] is the octant-o child of cell i:
- *   FF_CHILD_EMPTY                         empty sub-cell
+ * sorted by (first, level).  child[8*i + j], j = 0..7, are the sub-cells of cell i COMPACTED: the non-empty ones
+ * first, in octant order (0..7 = 4x + 2y + z), then FF_CHILD_EMPTY for the rest:
+ *   FF_CHILD_EMPTY                         no further sub-cell
  *   v >= 0                                 internal cell v
  *   (v & FF_CHILD_LEAF1) == FF_CHILD_LEAF1 and not MULTI: single-particle leaf, slot = v & FF_CHILD_SLOT
  *   FF_CHILD_MULTI set                     leaf with leaf_count[slot] > 1 particles starting at slot
@@ -270,6 +271,26 @@ int ff_get_launch_count(ff_ctx* ctx, uint64_t* launches);
  * measured ALU peak next to the nominal SMs x 128 x 2 x clock.
  */
 int ff_measure_fp32_peak(ff_ctx* ctx, int iters, double* tflops);
+
+/*
+ * The other FP32-pipe probes (same calling convention, result in TFLOP/s with an FMA counted as 2 flop):
+ * what the ALU roofline of ff_k_walk / ff_k_direct is measured against.
+ *   FF_PROBE_FFMA          the scalar FFMA chains of ff_measure_fp32_peak
+ *   FF_PROBE_FFMA2_PAIRS   packed FFMA2 with three distinct register-pair operands
+ *   FF_PROBE_FFMA2_REUSE   packed FFMA2 with one operand shared by consecutive instructions (operand reuse cache)
+ *   FF_PROBE_FFMA2_SCALAR  packed FFMA2 with one scalar operand in the broadcast form (how the sources enter Eq. 11-12)
+ *   FF_PROBE_EVAL          the evaluation loop of the walk alone: 38 packed FP32 instructions + 2 MUFU.RSQ per source
+ *                          and pair of targets on shared-memory records, 60 flop per interaction -- the ceiling of the
+ *                          walk and of the direct kernel
+ */
+enum {
+    FF_PROBE_FFMA = 0,
+    FF_PROBE_FFMA2_PAIRS = 1,
+    FF_PROBE_FFMA2_REUSE = 2,
+    FF_PROBE_FFMA2_SCALAR = 3,
+    FF_PROBE_EVAL = 4
+};
+int ff_measure_probe(ff_ctx* ctx, int kind, int iters, double* tflops);
 
 const char* ff_error_string(int code);
 /* Text of the last CUDA error seen by this context ("" if none). */

@@ -25,6 +25,7 @@ FF_ERR_INVALID_ARG, FF_ERR_WORKSPACE, FF_ERR_NO_TREE, FF_ERR_CAPACITY, FF_ERR_CU
 FF_OPT_THETA, FF_OPT_NLEAF, FF_OPT_COUNTERS, FF_OPT_TIMING, FF_OPT_GROUP = 1, 2, 3, 4, 5
 FF_N_PHASES = 7
 PHASES = ("bbox_keys", "sort", "build", "moments", "walk", "direct", "step")
+FF_PROBE_FFMA, FF_PROBE_FFMA2_PAIRS, FF_PROBE_FFMA2_REUSE, FF_PROBE_FFMA2_SCALAR, FF_PROBE_EVAL = 0, 1, 2, 3, 4
 FF_CHILD_EMPTY = -1
 FF_CHILD_LEAF1, FF_CHILD_MULTI, FF_CHILD_SLOT = 0x80000000, 0x40000000, 0x3FFFFFFF
 
@@ -32,7 +33,7 @@ FF_CHILD_LEAF1, FF_CHILD_MULTI, FF_CHILD_SLOT = 0x80000000, 0x40000000, 0x3FFFFF
 SYMBOLS = (
     "ff_workspace_bytes", "ff_create", "ff_destroy", "ff_set_stream", "ff_set_option", "ff_build_tree",
     "ff_eval_bh", "ff_eval_bh_range", "ff_eval_direct", "ff_eval_bh_host", "ff_eval_direct_host", "ff_step", "ff_get_tree",
-    "ff_get_timings", "ff_eval_bh_host_async", "ff_host_sync", "ff_get_counters", "ff_get_prefilter_count", "ff_get_launch_count", "ff_measure_fp32_peak", "ff_error_string",
+    "ff_get_timings", "ff_eval_bh_host_async", "ff_host_sync", "ff_get_counters", "ff_get_prefilter_count", "ff_get_launch_count", "ff_measure_fp32_peak", "ff_measure_probe", "ff_error_string",
     "ff_last_error",
 )
 
@@ -55,10 +56,11 @@ class ff_tree_view(ctypes.Structure):
                 ("cell_centre", ctypes.c_void_p), ("cell_moment", ctypes.c_void_p)]
 
 
-def shard_groups(n: int, world: int, rank: int):
-    """Target sharding of SURVEY.md 8(e): the walk groups (32 consecutive sorted targets) of an n-particle ensemble
-    split into `world` Morton-contiguous slices of equal size (+-1); returns (group_begin, group_end) of `rank`."""
-    groups = (n + 31) // 32
+def shard_groups(n: int, world: int, rank: int, group: int = 32):
+    """Target sharding of SURVEY.md 8(e): the walk groups (`group` consecutive sorted targets, FF_OPT_GROUP) of an
+    n-particle ensemble split into `world` Morton-contiguous slices of equal size (+-1); returns
+    (group_begin, group_end) of `rank`."""
+    groups = (n + group - 1) // group
     base, rem = divmod(groups, world)
     begin = rank * base + min(rank, rem)
     return begin, begin + base + (1 if rank < rem else 0)
@@ -119,6 +121,8 @@ def lib():
         L.ff_get_launch_count.argtypes = [vp, ctypes.POINTER(u64)]
         L.ff_measure_fp32_peak.restype = i32
         L.ff_measure_fp32_peak.argtypes = [vp, i32, ctypes.POINTER(f64)]
+        L.ff_measure_probe.restype = i32
+        L.ff_measure_probe.argtypes = [vp, i32, i32, ctypes.POINTER(f64)]
         L.ff_error_string.restype = ctypes.c_char_p
         L.ff_error_string.argtypes = [i32]
         L.ff_last_error.restype = ctypes.c_char_p
@@ -325,26 +329,8 @@ class FFContext:
         self._check(self._L.ff_measure_fp32_peak(self._h, int(iters), ctypes.byref(t)), "ff_measure_fp32_peak")
         return float(t.value)
 
-
-def canonical_tree(tree: dict):
-    """Canonical topology [(first, level, prefix, count, is_leaf)] sorted by (first, level) from
-    FFContext.get_tree(): the internal cells plus the leaf children they point to."""
-    key = tree["key"].astype("int64")
-    n, m = tree["n"], tree["n_cells"]
-    out = []
-    if m == 0:
-        return [(0, 0, 0, n, 1)]
-    first, end, level, child = tree["cell_first"], tree["cell_end"], tree["cell_level"], tree["child"]
-    for i in range(m):
-        f, l = int(first[i]), int(level[i])
-        out.append((f, l, int(key[f] >> (3 * (10 - l))), int(end[i]) - f, 0))
-        for o in range(8):
-            e = int(child[i, o])
-            if e == FF_CHILD_EMPTY or e >= 0:
-                continue
-            u = e & 0xFFFFFFFF
-            slot = u & FF_CHILD_SLOT
-            cnt = int(tree["leaf_count"][slot]) if (u & FF_CHILD_MULTI) else 1
-            out.append((slot, l + 1, int(key[slot] >> (3 * (10 - l - 1))), cnt, 1))
-    out.sort(key=lambda t: (t[0], t[1]))
-    return out
+    def measure_probe(self, kind: int, iters: int = 4096) -> float:
+        """ff_measure_probe: TFLOP/s of one of the FP32-pipe probes (FF_PROBE_*)."""
+        t = ctypes.c_double()
+        self._check(self._L.ff_measure_probe(self._h, int(kind), int(iters), ctypes.byref(t)), "ff_measure_probe")
+        return float(t.value)

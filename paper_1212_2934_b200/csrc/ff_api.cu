@@ -35,6 +35,7 @@ static size_t carve(ff_ctx* c, char* base, int64_t N)
     p = take(cap * 4);                            if (c) c->cell_end = (int32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_level = (int32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_list = (int32_t*)p;
+    p = take(cap * 16);                           if (c) c->cell_info = (int4*)p;
     p = take(cap * 32);                           if (c) c->cell_child = (int32_t*)p;
     p = take(cap * 16);                           if (c) c->cell_centre = (float4*)p;
     p = take(cap * 16);                           if (c) c->cell_moment = (float4*)p;
@@ -68,7 +69,7 @@ extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, 
     ff_ctx* c = new (std::nothrow) ff_ctx;
     if (!c) return FF_ERR_INVALID_ARG;
     memset(c, 0, sizeof(*c));
-    c->N = N; c->theta = theta; c->nleaf = 1;
+    c->N = N; c->theta = theta; c->nleaf = 1; c->group = 32;
     c->ws = (char*)workspace; c->ws_bytes = workspace_bytes;
     carve(c, c->ws, N);
     cudaError_t e = cudaGetDevice(&c->device);
@@ -131,7 +132,10 @@ extern "C" int ff_set_option(ff_ctx* c, int key, double value)
         return FF_OK;
     case FF_OPT_COUNTERS: c->count_enabled = value != 0.0; return FF_OK;
     case FF_OPT_TIMING: c->timing_enabled = value != 0.0; return FF_OK;
-    case FF_OPT_GROUP: return value == 32.0 ? FF_OK : FF_ERR_INVALID_ARG;
+    case FF_OPT_GROUP:
+        if (value != 32.0 && value != 64.0) return FF_ERR_INVALID_ARG;
+        c->group = (int)value;
+        return FF_OK;
     default: return FF_ERR_INVALID_ARG;
     }
 }
@@ -166,7 +170,7 @@ extern "C" int ff_eval_bh_range(ff_ctx* c, const float* pos, const float* mom, f
 {
     if (!c || !pos || !mom) return FF_ERR_INVALID_ARG;
     if (!c->tree_built) return FF_ERR_NO_TREE;
-    const int64_t groups = (c->n + 31) / 32;
+    const int64_t groups = (c->n + c->group - 1) / c->group;
     if (group_end < 0) group_end = groups;
     if (group_begin < 0 || group_begin > group_end || group_end > groups) return FF_ERR_INVALID_ARG;
     int rc;
@@ -354,7 +358,13 @@ extern "C" int ff_get_launch_count(ff_ctx* c, uint64_t* launches)
 extern "C" int ff_measure_fp32_peak(ff_ctx* c, int iters, double* tflops)
 {
     if (!c || !tflops) return FF_ERR_INVALID_ARG;
-    return ff_launch_fp32_peak(c, iters, tflops);
+    return ff_launch_probe(c, FF_PROBE_FFMA, iters, tflops);
+}
+
+extern "C" int ff_measure_probe(ff_ctx* c, int kind, int iters, double* tflops)
+{
+    if (!c || !tflops) return FF_ERR_INVALID_ARG;
+    return ff_launch_probe(c, kind, iters, tflops);
 }
 
 extern "C" const char* ff_error_string(int code)

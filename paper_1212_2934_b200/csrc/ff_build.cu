@@ -59,7 +59,8 @@ __device__ __forceinline__ int ff_gallop_bound(const uint32_t* __restrict__ key,
 //            its first slot and level; level histogram
 //   phase 3  eight lanes per cell: lane o finds the end of octant o with a galloping search in
 //            the sorted keys (one search per lane, all of similar length), which gives the cell's
-//            range and its eight child links; the cell's id is appended to its level's list
+//            range and its child links (non-empty sub-cells compacted to the front, in octant
+//            order); the cell's id is appended to its level's list
 //            (ff_k_moments walks the levels deepest first)
 // The paper builds the tree by locked insertion (kernel 2); no locks here, and
 // the result does not depend on scheduling except for the order inside a level list, which no
@@ -67,8 +68,8 @@ __device__ __forceinline__ int ff_gallop_bound(const uint32_t* __restrict__ key,
 __global__ void __launch_bounds__(FF_BUILD_THREADS)
 ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restrict__ blk,
            int32_t* __restrict__ cell_base, int32_t* __restrict__ cell_first, int32_t* __restrict__ cell_end,
-           int32_t* __restrict__ cell_level, int32_t* __restrict__ cell_child, int32_t* __restrict__ leaf_count,
-           int32_t* __restrict__ cell_list, int cell_cap, ff_globals* g)
+           int32_t* __restrict__ cell_level, int32_t* __restrict__ cell_child, int4* __restrict__ cell_info,
+           int32_t* __restrict__ leaf_count, int32_t* __restrict__ cell_list, int cell_cap, ff_globals* g)
 {
     cg::grid_group grid = cg::this_grid();
     __shared__ uint32_t wsum[FF_BUILD_THREADS / 32];
@@ -204,8 +205,14 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
         else if (cc > nleaf && l + 1 < FF_MAX_LEVEL) ent = cell_base[b] + (l - ff_lprev(key, b));   // internal child: level l+1 at slot b
         else if (cc == 1) ent = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)b);
         else { ent = (int32_t)(FF_CHILD_LEAF1 | FF_CHILD_MULTI | (uint32_t)b); leaf_count[b] = cc; }
-        cell_child[8 * (size_t)id + o] = ent;
-        if (o == 7) cell_end[id] = e;
+        // the eight links are stored COMPACTED: the non-empty sub-cells first, in octant order, then the empty ones
+        // (the walk pushes the first n_children links without looking at them; the moments add them in this order)
+        const int gsh = threadIdx.x & 24;
+        const unsigned present = (__ballot_sync(gmask, cc != 0) >> gsh) & 0xffu;
+        const int nch = __popc(present);
+        const int rank = __popc(present & ((1u << o) - 1u));
+        cell_child[8 * (size_t)id + (cc != 0 ? rank : nch + (o - rank))] = ent;
+        if (o == 7) { cell_end[id] = e; cell_info[id] = make_int4(first, e, nch, l); }
         if (o == 0) cell_list[atomicAdd(&s_cur[l], 1)] = id;
     }
 }
@@ -322,7 +329,7 @@ int ff_launch_build(ff_ctx* c)
     int nleaf = c->nleaf, cap = (int)c->cell_cap;
     void* args[] = { (void*)&c->key[0], (void*)&n, (void*)&nleaf, (void*)&c->scan_blk, (void*)&c->cell_base,
                      (void*)&c->cell_first, (void*)&c->cell_end, (void*)&c->cell_level, (void*)&c->cell_child,
-                     (void*)&c->leaf_count, (void*)&c->cell_list, (void*)&cap, (void*)&c->g };
+                     (void*)&c->cell_info, (void*)&c->leaf_count, (void*)&c->cell_list, (void*)&cap, (void*)&c->g };
     FF_CUDA(c, cudaLaunchCooperativeKernel((const void*)ff_k_build, dim3(blocks), dim3(FF_BUILD_THREADS), args, 0,
                                            c->stream));
     c->launches++;

@@ -36,8 +36,8 @@
 #define FF_WALK_STACK 1024         // traversal stack entries per warp
 #define FF_WALK_PEND 64            // pending interaction ring per warp (two batches of 32)
 #ifndef FF_WALK_PROBE_PAIRS
-#define FF_WALK_PROBE_PAIRS 2      // probe members (x2) of the opening pre-filter, taken in the order: the members
-#endif                             // at the x, y, z extremes of the group's box, then the first and the last member
+#define FF_WALK_PROBE_PAIRS 2      // probe members (x2) of the opening pre-filter: the members at the x and y extremes
+#endif                             // of the group's box
 #define FF_WALK_AMB_ROOM 256       // stack room an ambiguous-queue round may need (32 cells x 8 children)
 
 // ---- direct geometry (ff_direct.cu) -------------------------------------------
@@ -75,7 +75,8 @@ struct ff_ctx {
     int moments_valid;
     int device;
     int num_sms;
-    int occ_walk[2], occ_build, occ_moments;   // resident blocks per SM of the persistent / cooperative kernels (0 = not queried yet)
+    int group;                // targets per walk group W: 32 or 64 (FF_OPT_GROUP)
+    int occ_walk[8], occ_build, occ_moments;   // resident blocks per SM of the persistent / cooperative kernels (0 = not queried yet)
     cudaStream_t stream;
     // pipelined *_host calls: uploads on in_stream, compute on `stream`, downloads on out_stream, staging
     // buffers and events double-buffered by call parity (ff_api.cu)
@@ -95,6 +96,7 @@ struct ff_ctx {
     uint32_t* scan_blk;               // block sums of the scan
     uint32_t* sort_status;            // [FF_SORT_PASSES][n_tiles][FF_RADIX] look-back status words
     int32_t *cell_first, *cell_end, *cell_level;
+    int4* cell_info;                  // [cap] first, end, number of children, level: what the walk reads per cell
     int32_t* cell_list;               // [cap] cell ids grouped by level
     int32_t* cell_child;              // [cap][8]
     float4 *cell_centre, *cell_moment;
@@ -147,7 +149,7 @@ int ff_launch_moments(ff_ctx* c, const float* mom);
 int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out, int group_begin = 0, int group_end = -1);
 int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n, float* H_out, float* F_out,
                      float lj_eps = 0.0f, float lj_sigma = 1.0f, float lj_cutoff = 0.0f);   // lj_eps != 0: F_out = f^dip + f^sr
-int ff_launch_fp32_peak(ff_ctx* c, int iters, double* tflops);
+int ff_launch_probe(ff_ctx* c, int kind, int iters, double* tflops);
 int ff_launch_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n,
                    const ff_step_params* p, uint64_t step_index);
 

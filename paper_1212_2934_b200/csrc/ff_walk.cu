@@ -4,23 +4,25 @@
 // spatially close particles and "the first thread of a warp" fetches cell data to
 // shared memory.  That design (one cell per step, broadcast to 32 lanes) leaves
 // the FP32 pipe idle during every dependent cell fetch.  Here a warp owns one
-// GROUP of 32 consecutive sorted targets and splits the work in two:
+// GROUP of W consecutive sorted targets (W = 32 by default, 64 as an option:
+// DESIGN.md reading Q2) and splits the work in two:
 //
 //   list building  -- each LANE pops a DIFFERENT stack entry, tests it against the
 //                     whole group (opening rule O5 of DESIGN.md) and either appends
 //                     it to a shared-memory interaction ring or pushes its children;
 //                     traversal cost is amortised over 32 entries per round.
 //   evaluation     -- whenever 32 interactions are pending every lane evaluates them
-//                     for its OWN target: a dense, branch-free loop of Eq. 11 / Eq. 12
-//                      fed by broadcast float4 shared-memory reads.
+//                     for its OWN TWO targets: a dense, branch-free loop of Eq. 11 /
+//                     Eq. 12 fed by broadcast shared-memory reads.
 //
 // Blackwell specific: the evaluation and the opening test are written with the
 // packed FP32 instructions of sm_100 (FFMA2 / FMUL2 / FADD2 through __ffma2_rn,
-// __fmul2_rn, __fadd2_rn): one lane handles TWO sources (or two group members)
-// per instruction.  The FP32 pipe does the same work, but it needs half the
-// issue slots, and issue was the limiter of the scalar version (profiles/).  The
-// ring therefore stores sources as PAIRS: (x0,x1,y0,y1) (z0,z1,mx0,mx1)
-// (my0,my1,mz0,mz1), three broadcast LDS.128 per two sources.
+// __fmul2_rn, __fadd2_rn).  Every lane holds TWO targets in the halves of its
+// register pairs and evaluates one source against both per instruction
+// (ff_pair.cuh).  W = 32: lanes l and l + 16 hold the same two targets (l, l + 16)
+// and split the sources of a batch between them (even / odd ring entries); the
+// two partial sums are added with one shuffle per accumulator at the end.
+// W = 64: lane l holds targets l and l + 32 and every lane evaluates every source.
 //
 // Both phases produce exactly the interaction set of the oracle's recursive walk;
 // only the summation order differs.  fp32 arithmetic; the opening test uses
@@ -29,146 +31,155 @@
 #include "ff_internal.cuh"
 #include "ff_pair.cuh"
 
-#define FF_PEND_PAIRS (FF_WALK_PEND / 2)
-
+template <int W>
 struct ff_walk_smem {
     int32_t stack[FF_WALK_STACK];
-    float4 pend[FF_PEND_PAIRS * 3];    // pair p: [3p] = x0,x1,y0,y1  [3p+1] = z0,z1,mx0,mx1  [3p+2] = my0,my1,mz0,mz1
-    float4 mem_xy[16];                 // group members, pair m: x0,x1,y0,y1
-    float2 mem_z[16];                  //                        z0,z1
+    float4 pendA[FF_WALK_PEND];        // ring entry e: x, y, z, mx
+    float2 pendB[FF_WALK_PEND];        //               my, mz
+    float4 mem_xy[W / 2];              // group members in pairs for the opening test, pair m: x0,x1,y0,y1
+    float2 mem_z[W / 2];               //                                                   z0,z1
     float4 probe_xy[FF_WALK_PROBE_PAIRS];   // probe members of the opening pre-filter, same pair layout
     float2 probe_z[FF_WALK_PROBE_PAIRS];
     float4 bb_lo, bb_hi;               // bounding box of the group's members (exact min / max)
     int32_t amb[64];                   // cells the pre-filter could not decide, waiting for the full test
 };
 
-// write one interaction (A = position, B = moment) to ring slot `slot`
-__device__ __forceinline__ void ff_ring_store(ff_walk_smem& sm, int slot, const float4& A, const float4& B)
-{
-    float* f = reinterpret_cast<float*>(sm.pend) + (slot >> 1) * 12 + (slot & 1);
-    f[0] = A.x; f[2] = A.y; f[4] = A.z; f[6] = B.x; f[8] = B.y; f[10] = B.z;
-}
-
-// one group of 32 consecutive sorted targets, walked by one warp
-template <bool COUNT>
+// one group of W consecutive sorted targets, walked by one warp
+template <int W, bool COUNT, bool BUCKET>
 __device__ __forceinline__ void
-ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
+ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
           int n, float theta, const int n_cells, const float4* __restrict__ pos_s,
           const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
-          const int32_t* __restrict__ cell_first,
-          const int32_t* __restrict__ cell_end, const int4* __restrict__ cell_child,
+          const int4* __restrict__ cell_info, const int4* __restrict__ cell_child,
           const int32_t* __restrict__ leaf_count, const float4* __restrict__ centre,
           const float4* __restrict__ moment, float* __restrict__ H_out, float* __restrict__ F_out,
           unsigned long long* __restrict__ counters)
 {
-    const int g0 = grp * 32;
-    const int g1 = min(n, g0 + 32);
+    constexpr int ST = (W == 32) ? 2 : 1;                  // ring entries per evaluation step of one lane
+    constexpr int BATCH_ITERS = 32 / ST;                   // evaluation steps per batch of 32 ring entries
+    const int g0 = grp * W;
+    const int g1 = min(n, g0 + W);
     const int nm = g1 - g0;
     const unsigned lt = (1u << lane) - 1u;
+    const int half = (W == 32) ? (lane >> 4) : 0;          // W = 32: this lane takes the even (0) or odd (1) entries
+    const int i0 = (W == 32) ? (lane & 15) : lane;         // member indices of the lane's two targets
+    const int i1 = i0 + W / 2;
 
-    // own target (lanes past the end duplicate the last member; their results are dropped)
-    const int k = g0 + min(lane, nm - 1);
-    const float4 pk = __ldg(pos_s + k), uk = __ldg(mom_s + k);
+    // own targets (members past a ragged end duplicate the last member; their results are dropped)
+    const int k0 = g0 + min(i0, nm - 1), k1 = g0 + min(i1, nm - 1);
+    const float4 p0 = __ldg(pos_s + k0), u0 = __ldg(mom_s + k0);
+    const float4 p1 = __ldg(pos_s + k1), u1 = __ldg(mom_s + k1);
     ff_target2 tg;
-    tg.px = ff_dup(pk.x); tg.py = ff_dup(pk.y); tg.pz = ff_dup(pk.z);
-    tg.ux = ff_dup(uk.x); tg.uy = ff_dup(uk.y); tg.uz = ff_dup(uk.z);
+    tg.px = make_float2(p0.x, p1.x); tg.py = make_float2(p0.y, p1.y); tg.pz = make_float2(p0.z, p1.z);
+    tg.ux = make_float2(u0.x, u1.x); tg.uy = make_float2(u0.y, u1.y); tg.uz = make_float2(u0.z, u1.z);
     ff_acc2 s;
-    s.hx = s.hy = s.hz = s.fx = s.fy = s.fz = s.sk = ff_dup(0.0f);
+    ff_acc2_zero(s);
     unsigned long long c_cell = 0, c_part = 0, c_mac = 0, c_amb = 0;
 
-    {   // group members in pair layout for the opening test; the ring's first batch = the members themselves
-        float* mxy = reinterpret_cast<float*>(sm.mem_xy) + (lane >> 1) * 4 + (lane & 1);
-        mxy[0] = pk.x; mxy[2] = pk.y;
-        reinterpret_cast<float*>(sm.mem_z)[lane] = pk.z;
-        ff_ring_store(sm, lane, pk, uk);
-        // pre-filter data: exact bounding box of the members and the probe members (the members that
-        // attain the box extremes -- chosen on a key that trades the 5 low bits for the lane --, the
-        // first and the last).  Lanes past a ragged end hold copies of the last member, which is harmless.
-        const uint32_t ox = ff_f2ord(pk.x), oy = ff_f2ord(pk.y), oz = ff_f2ord(pk.z);
-        const float lox = ff_ord2f(__reduce_min_sync(FF_FULL, ox)), hix = ff_ord2f(__reduce_max_sync(FF_FULL, ox));
-        const float loy = ff_ord2f(__reduce_min_sync(FF_FULL, oy)), hiy = ff_ord2f(__reduce_max_sync(FF_FULL, oy));
-        const float loz = ff_ord2f(__reduce_min_sync(FF_FULL, oz)), hiz = ff_ord2f(__reduce_max_sync(FF_FULL, oz));
+    {   // group members in pair layout for the opening test; the ring's first batch(es) = the members themselves
+        auto put_member = [&](int i, const float4& p, const float4& u) {
+            float* mxy = reinterpret_cast<float*>(sm.mem_xy) + (i >> 1) * 4 + (i & 1);
+            mxy[0] = p.x; mxy[2] = p.y;
+            reinterpret_cast<float*>(sm.mem_z)[i] = p.z;
+            sm.pendA[i] = make_float4(p.x, p.y, p.z, u.x);
+            sm.pendB[i] = make_float2(u.y, u.z);
+        };
+        if (W == 32) {
+            put_member(lane, half ? p1 : p0, half ? u1 : u0);
+        } else {
+            put_member(i0, p0, u0);
+            put_member(i1, p1, u1);
+        }
+        // pre-filter data: exact bounding box of the members and the probe members (the members that attain the x
+        // and y extremes of the box, chosen on a key that trades the low bits for the member index).  Members past
+        // a ragged end are copies of the last member, which is harmless.
+        const uint32_t ox = min(ff_f2ord(p0.x), ff_f2ord(p1.x)), oy = min(ff_f2ord(p0.y), ff_f2ord(p1.y)),
+                       oz = min(ff_f2ord(p0.z), ff_f2ord(p1.z));
+        const uint32_t Ox = max(ff_f2ord(p0.x), ff_f2ord(p1.x)), Oy = max(ff_f2ord(p0.y), ff_f2ord(p1.y)),
+                       Oz = max(ff_f2ord(p0.z), ff_f2ord(p1.z));
+        const float lox = ff_ord2f(__reduce_min_sync(FF_FULL, ox)), hix = ff_ord2f(__reduce_max_sync(FF_FULL, Ox));
+        const float loy = ff_ord2f(__reduce_min_sync(FF_FULL, oy)), hiy = ff_ord2f(__reduce_max_sync(FF_FULL, Oy));
+        const float loz = ff_ord2f(__reduce_min_sync(FF_FULL, oz)), hiz = ff_ord2f(__reduce_max_sync(FF_FULL, Oz));
         if (lane == 0) {
             sm.bb_lo = make_float4(lox, loy, loz, 0.f);
             sm.bb_hi = make_float4(hix, hiy, hiz, 0.f);
         }
-        const uint32_t kx = (ox & ~31u) | lane, ky = (oy & ~31u) | lane, kz = (oz & ~31u) | lane;
-        int src[8];
-        src[0] = __reduce_min_sync(FF_FULL, kx) & 31; src[1] = __reduce_max_sync(FF_FULL, kx) & 31;
-        src[2] = __reduce_min_sync(FF_FULL, ky) & 31; src[3] = __reduce_max_sync(FF_FULL, ky) & 31;
-        src[4] = __reduce_min_sync(FF_FULL, kz) & 31; src[5] = __reduce_max_sync(FF_FULL, kz) & 31;
-        src[6] = 0; src[7] = 31;
-#pragma unroll
-        for (int t = 0; t < 2 * FF_WALK_PROBE_PAIRS; ++t)
-            if (lane == src[t]) {
-                float* f = reinterpret_cast<float*>(sm.probe_xy) + (t >> 1) * 4 + (t & 1);
-                f[0] = pk.x; f[2] = pk.y;
-                reinterpret_cast<float*>(sm.probe_z)[t] = pk.z;
-            }
+        static_assert(FF_WALK_PROBE_PAIRS == 2, "four probe members: the x and y extremes");
+        constexpr uint32_t IM = W - 1;                     // member index in the low bits of the key
+        auto key = [&](float a, int i) { return (ff_f2ord(a) & ~IM) | (uint32_t)i; };
+        const int s0 = __reduce_min_sync(FF_FULL, min(key(p0.x, i0), key(p1.x, i1))) & IM;
+        const int s1 = __reduce_max_sync(FF_FULL, max(key(p0.x, i0), key(p1.x, i1))) & IM;
+        const int s2 = __reduce_min_sync(FF_FULL, min(key(p0.y, i0), key(p1.y, i1))) & IM;
+        const int s3 = __reduce_max_sync(FF_FULL, max(key(p0.y, i0), key(p1.y, i1))) & IM;
+        __syncwarp();
+        if (lane < 2 * FF_WALK_PROBE_PAIRS) {
+            const int m = lane == 0 ? s0 : lane == 1 ? s1 : lane == 2 ? s2 : s3;
+            const float* mxy = reinterpret_cast<const float*>(sm.mem_xy) + (m >> 1) * 4 + (m & 1);
+            float* f = reinterpret_cast<float*>(sm.probe_xy) + (lane >> 1) * 4 + (lane & 1);
+            f[0] = mxy[0]; f[2] = mxy[2];
+            reinterpret_cast<float*>(sm.probe_z)[lane] = reinterpret_cast<const float*>(sm.mem_z)[m];
+        }
     }
     __syncwarp();
     // the group's own members: direct terms, self skipped by index (Alg. 1 line 5);
     // slots >= nm of a ragged last group hold copies of the last member and are masked the same way
 #pragma unroll 2
-    for (int jj = 0; jj < 16; ++jj) {
-        const float4 q0 = sm.pend[3 * jj], q1 = sm.pend[3 * jj + 1], q2 = sm.pend[3 * jj + 2];
+    for (int jj = 0; jj < W / ST; ++jj) {
+        const int j = ST * jj + half;
+        const float4 A = sm.pendA[j];
+        const float2 B = sm.pendB[j];
         float2 dx, dy, dz, r2;
-        ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
+        ff_pair2_geom(A, tg, dx, dy, dz, r2);
         float2 rinv;
-        rinv.x = (2 * jj == lane || 2 * jj >= nm) ? 0.0f : ff_rsqrt(r2.x);
-        rinv.y = (2 * jj + 1 == lane || 2 * jj + 1 >= nm) ? 0.0f : ff_rsqrt(r2.y);
-        ff_pair2_accum(q1, q2, tg, dx, dy, dz, rinv, s);
+        rinv.x = (j == i0 || j >= nm) ? 0.0f : ff_rsqrt(r2.x);
+        rinv.y = (j == i1 || j >= nm) ? 0.0f : ff_rsqrt(r2.y);
+        ff_pair2_accum(A, B, tg, dx, dy, dz, rinv, s);
     }
     if (COUNT) c_part += (unsigned long long)nm * (unsigned long long)(nm - 1);
     __syncwarp();
 
     const float th2 = __fmul_rn(theta, theta);
-    int pend_head = 0, pend_cnt = 0;                       // warp-uniform ring state (entries)
+    int pend_head = 0, pend_cnt = 0;                       // warp-uniform ring state (entries); head is 0 or 32
     int sp_top = 0;                                        // warp-uniform stack size
 
-    // evaluate `pairs` pending source pairs starting at ring entry pend_head for this lane's target
-    auto eval = [&](int pairs) {
+    // evaluate `iters` steps of this lane starting at ring entry pend_head (W = 32: entries head + 2 i + half)
+    auto eval = [&](int iters) {
         __syncwarp();
-        const float4* q = sm.pend + 3 * (pend_head >> 1);
-        if (pairs == 16) {
+        const float4* qa = sm.pendA + pend_head + half;
+        const float2* qb = sm.pendB + pend_head + half;
+        if (iters == BATCH_ITERS) {
 #pragma unroll 4
-            for (int jj = 0; jj < 16; ++jj) {
-                const float4 q0 = q[3 * jj], q1 = q[3 * jj + 1], q2 = q[3 * jj + 2];
-                float2 dx, dy, dz, r2;
-                ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
-                ff_pair2_accum(q1, q2, tg, dx, dy, dz, make_float2(ff_rsqrt(r2.x), ff_rsqrt(r2.y)), s);
-            }
+            for (int i = 0; i < BATCH_ITERS; ++i) ff_pair2(qa[ST * i], qb[ST * i], tg, s);
         } else {
-            for (int jj = 0; jj < pairs; ++jj) {
-                const float4 q0 = q[3 * jj], q1 = q[3 * jj + 1], q2 = q[3 * jj + 2];
-                float2 dx, dy, dz, r2;
-                ff_pair2_geom(q0, q1, tg, dx, dy, dz, r2);
-                ff_pair2_accum(q1, q2, tg, dx, dy, dz, make_float2(ff_rsqrt(r2.x), ff_rsqrt(r2.y)), s);
-            }
+            for (int i = 0; i < iters; ++i) ff_pair2(qa[ST * i], qb[ST * i], tg, s);
         }
         __syncwarp();
     };
-    // append the lanes with `take` set (data A = position, B = moment) to the ring
-    auto append = [&](bool take, const float4& A, const float4& B) {
-        unsigned m = __ballot_sync(FF_FULL, take);
-        if (take) ff_ring_store(sm, (pend_head + pend_cnt + __popc(m & lt)) & (FF_WALK_PEND - 1), A, B);
+    // append the lanes with `take` set (A = x, y, z, mx; B = my, mz) to the ring
+    auto append = [&](bool take, const float4& A, const float2& B) {
+        const unsigned m = __ballot_sync(FF_FULL, take);
+        if (take) {
+            const int slot = (pend_head + pend_cnt + __popc(m & lt)) & (FF_WALK_PEND - 1);
+            sm.pendA[slot] = A;
+            sm.pendB[slot] = B;
+        }
         pend_cnt += __popc(m);
     };
     auto drain = [&]() {
         while (pend_cnt >= 32) {
-            eval(16);
-            pend_head = (pend_head + 32) & (FF_WALK_PEND - 1);
+            eval(BATCH_ITERS);
+            pend_head ^= 32;
             pend_cnt -= 32;
         }
     };
-    // a leaf with several particles (depth cap or N_leaf > 1): the warp streams it through the ring
+    // a leaf with several particles (depth cap, or N_leaf > 8): the warp streams it through the ring
     auto coop_leaf = [&](int first, int cnt) {
         for (int base = first; base < first + cnt; base += 32) {
-            int j = base + lane;
-            bool ok = j < first + cnt && !(j >= g0 && j < g1);
+            const int j = base + lane;
+            const bool ok = j < first + cnt && !(j >= g0 && j < g1);
             float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = A;
             if (ok) { A = __ldg(pos_s + j); B = __ldg(mom_s + j); }
-            append(ok, A, B);
+            append(ok, make_float4(A.x, A.y, A.z, B.x), make_float2(B.y, B.z));
             if (COUNT) c_part += (unsigned long long)__popc(__ballot_sync(FF_FULL, ok)) * nm;
             drain();
         }
@@ -186,7 +197,7 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
     while (sp_top > 0 || amb_cnt > 0) {
         // Source of this round's entries.  Normal round: pop the stack, decide cells with the cheap
         // pre-filter, park the undecided ones in sm.amb.  Ambiguous round (32 parked, or the stack ran
-        // dry): full 32-member test on parked cells.  Stack nearly full: pop one entry at a time as
+        // dry): full W-member test on parked cells.  Stack nearly full: pop one entry at a time as
         // before; parked cells wait (and, if 32 are parked already, popped cells get the full test).
         const int room = FF_WALK_STACK - 80 - sp_top;
         const bool amb_round = sp_top == 0 || (amb_cnt >= 32 && room >= FF_WALK_AMB_ROOM);
@@ -204,14 +215,14 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
         }
         __syncwarp();
         const bool is_cell = e >= 0;
-        const bool is_part = !is_cell && e != FF_CHILD_EMPTY && !((uint32_t)e & FF_CHILD_MULTI);
-        const bool is_multi = !is_cell && e != FF_CHILD_EMPTY && ((uint32_t)e & FF_CHILD_MULTI);
+        const bool is_leaf = !is_cell && e != FF_CHILD_EMPTY;
+        const bool is_multi = is_leaf && ((uint32_t)e & FF_CHILD_MULTI);
+        const bool is_part = is_leaf && !is_multi;
         const int slot = (int)((uint32_t)e & FF_CHILD_SLOT);
         float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = A;
-        int first = 0, end = 0;
+        int4 info = make_int4(0, 0, 0, 0);                 // first, end, number of children
         if (is_cell) {
-            A = __ldg(centre + e); B = __ldg(moment + e);
-            if (!amb_round) { first = __ldg(cell_first + e); end = __ldg(cell_end + e); }
+            A = __ldg(centre + e); B = __ldg(moment + e); info = __ldg(cell_info + e);
         } else if (is_part) {
             A = __ldg(pos_s + slot); B = __ldg(mom_s + slot);
         }
@@ -223,7 +234,7 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
         if (full) {
             float d2min = 3.0e38f;
 #pragma unroll 8
-            for (int m = 0; m < 16; ++m) {
+            for (int m = 0; m < W / 2; ++m) {
                 const float4 qxy = sm.mem_xy[m];
                 const float2 qz = sm.mem_z[m];
                 const float2 dx = __fadd2_rn(make_float2(qxy.x, qxy.y), nax);
@@ -258,7 +269,7 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
             }
             amb = !acc && (A.w < __fmul_rn(th2, d2min));
         }
-        const bool holds = first < g1 && end > g0;         // the cell's range holds a member: always open (Q3)
+        const bool holds = info.x < g1 && info.y > g0;     // the cell's range holds a member: always open (Q3)
         const bool tested = is_cell && !holds;
         const bool accept_cell = tested && acc;
         const bool park = tested && amb;
@@ -275,71 +286,88 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
             if (park) sm.amb[amb_cnt + __popc(pm & lt)] = e;
             amb_cnt += __popc(pm);
         }
-        append(take, A, B);
+        append(take, make_float4(A.x, A.y, A.z, B.x), make_float2(B.y, B.z));
+        // the children of an opened cell: the non-empty sub-cells, compacted to the front of its eight links
         int4 c0 = make_int4(-1, -1, -1, -1), c1 = c0;
-        if (open) { c0 = __ldg(cell_child + 2 * (size_t)e); c1 = __ldg(cell_child + 2 * (size_t)e + 1); }
+        int nch = 0;
+        if (open) {
+            c0 = __ldg(cell_child + 2 * (size_t)e); c1 = __ldg(cell_child + 2 * (size_t)e + 1);
+            nch = info.z;
+        }
         const int lcnt = is_multi ? __ldg(leaf_count + slot) : 0;
         drain();                                           // overlaps the child loads
-        // a bucket leaf of up to eight particles (N_leaf > 1) is expanded like an opened cell: its particles go
-        // back on the stack as single-particle entries and are handled 32 at a time in the coming rounds
-        const bool small_leaf = is_multi && lcnt <= 8;
-        if (small_leaf) {
-            const int32_t p0 = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)slot);
-            c0 = make_int4(p0, lcnt > 1 ? p0 + 1 : -1, lcnt > 2 ? p0 + 2 : -1, lcnt > 3 ? p0 + 3 : -1);
-            c1 = make_int4(lcnt > 4 ? p0 + 4 : -1, lcnt > 5 ? p0 + 5 : -1, lcnt > 6 ? p0 + 6 : -1, lcnt > 7 ? p0 + 7 : -1);
+        bool stream_leaf = is_multi;
+        if (BUCKET) {
+            // a bucket leaf of up to eight particles (N_leaf > 1) is expanded like an opened cell: its particles go
+            // back on the stack as single-particle entries and are handled 32 at a time in the coming rounds
+            if (is_multi && lcnt <= 8) {
+                const int32_t q0 = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)slot);
+                c0 = make_int4(q0, q0 + 1, q0 + 2, q0 + 3);
+                c1 = make_int4(q0 + 4, q0 + 5, q0 + 6, q0 + 7);
+                nch = lcnt;
+                stream_leaf = false;
+            }
         }
         // push the children of the opened cells
-        int nch = (c0.x != -1) + (c0.y != -1) + (c0.z != -1) + (c0.w != -1) + (c1.x != -1) + (c1.y != -1) +
-                  (c1.z != -1) + (c1.w != -1);
         int incl = nch;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(FF_FULL, incl, o); if (lane >= o) incl += y; }
-        int total = __shfl_sync(FF_FULL, incl, 31);
-        if (nch) {
-            int wpos = sp_top + incl - nch;
-            if (c0.x != -1) sm.stack[wpos++] = c0.x;
-            if (c0.y != -1) sm.stack[wpos++] = c0.y;
-            if (c0.z != -1) sm.stack[wpos++] = c0.z;
-            if (c0.w != -1) sm.stack[wpos++] = c0.w;
-            if (c1.x != -1) sm.stack[wpos++] = c1.x;
-            if (c1.y != -1) sm.stack[wpos++] = c1.y;
-            if (c1.z != -1) sm.stack[wpos++] = c1.z;
-            if (c1.w != -1) sm.stack[wpos++] = c1.w;
+        const int total = __shfl_sync(FF_FULL, incl, 31);
+        {
+            int32_t* w = sm.stack + (sp_top + incl - nch);
+            if (nch > 0) w[0] = c0.x;
+            if (nch > 1) w[1] = c0.y;
+            if (nch > 2) w[2] = c0.z;
+            if (nch > 3) w[3] = c0.w;
+            if (nch > 4) w[4] = c1.x;
+            if (nch > 5) w[5] = c1.y;
+            if (nch > 6) w[6] = c1.z;
+            if (nch > 7) w[7] = c1.w;
         }
         sp_top += total;
         // multi-particle leaves met this round
-        unsigned mm = __ballot_sync(FF_FULL, is_multi && !small_leaf);
+        unsigned mm = __ballot_sync(FF_FULL, stream_leaf);
         while (mm) {
-            int src = __ffs(mm) - 1;
+            const int src = __ffs(mm) - 1;
             mm &= mm - 1;
             coop_leaf(__shfl_sync(FF_FULL, slot, src), __shfl_sync(FF_FULL, lcnt, src));
         }
         __syncwarp();
     }
     if (pend_cnt > 0) {
-        // pad an odd tail with a copy of the last entry's position carrying a zero moment: every term
-        // of Eq. 11-12 is linear in u_j, so the pad contributes exactly 0 and stays finite
-        if (pend_cnt & 1) {
+        // W = 32: the two half-warps take the even / odd entries; an odd tail is padded with a copy of the last
+        // entry's position carrying a zero moment: every term of Eq. 11-12 is linear in u_j, so the pad contributes
+        // exactly 0 and stays finite
+        if (W == 32 && (pend_cnt & 1)) {
             __syncwarp();
             if (lane == 0) {
-                const float* f = reinterpret_cast<const float*>(sm.pend);
-                int last = (pend_head + pend_cnt - 1) & (FF_WALK_PEND - 1);
-                const float* src = f + (last >> 1) * 12 + (last & 1);
-                float4 A = make_float4(src[0], src[2], src[4], 0.f);
-                ff_ring_store(sm, (last + 1) & (FF_WALK_PEND - 1), A, make_float4(0.f, 0.f, 0.f, 0.f));
+                const float4 last = sm.pendA[pend_head + pend_cnt - 1];
+                sm.pendA[pend_head + pend_cnt] = make_float4(last.x, last.y, last.z, 0.f);
+                sm.pendB[pend_head + pend_cnt] = make_float2(0.f, 0.f);
             }
         }
-        eval((pend_cnt + 1) >> 1);
+        eval((pend_cnt + ST - 1) / ST);
     }
 
-    if (lane < nm) {
-        // fold the even / odd halves; f = fv + sk u_k
-        const float sk = s.sk.x + s.sk.y;
-        const float fx = fmaf(sk, uk.x, s.fx.x + s.fx.y), fy = fmaf(sk, uk.y, s.fy.x + s.fy.y),
-                    fz = fmaf(sk, uk.z, s.fz.x + s.fz.y);
-        size_t o = (size_t)__ldg(perm + k) * 3;            // a7: back to caller order
-        if (H_out) { H_out[o] = s.hx.x + s.hx.y; H_out[o + 1] = s.hy.x + s.hy.y; H_out[o + 2] = s.hz.x + s.hz.y; }
-        if (F_out) { F_out[o] = fx; F_out[o + 1] = fy; F_out[o + 2] = fz; }
+    // W = 32: lanes l and l + 16 hold partial sums of the same two targets
+    if (W == 32) {
+#define FF_FOLD(v) v.x += __shfl_xor_sync(FF_FULL, v.x, 16); v.y += __shfl_xor_sync(FF_FULL, v.y, 16)
+        FF_FOLD(s.hx); FF_FOLD(s.hy); FF_FOLD(s.hz); FF_FOLD(s.fx); FF_FOLD(s.fy); FF_FOLD(s.fz); FF_FOLD(s.sk);
+#undef FF_FOLD
+    }
+    auto store = [&](int k, const float4& uk, float hx, float hy, float hz, float fvx, float fvy, float fvz, float sk) {
+        const size_t o = (size_t)__ldg(perm + k) * 3;      // a7: back to caller order;  f = fv + sk u_k
+        if (H_out) { H_out[o] = hx; H_out[o + 1] = hy; H_out[o + 2] = hz; }
+        if (F_out) { F_out[o] = fmaf(sk, uk.x, fvx); F_out[o + 1] = fmaf(sk, uk.y, fvy); F_out[o + 2] = fmaf(sk, uk.z, fvz); }
+    };
+    if (W == 32) {
+        if (lane < nm) {
+            if (half) store(k1, u1, s.hx.y, s.hy.y, s.hz.y, s.fx.y, s.fy.y, s.fz.y, s.sk.y);
+            else store(k0, u0, s.hx.x, s.hy.x, s.hz.x, s.fx.x, s.fy.x, s.fz.x, s.sk.x);
+        }
+    } else {
+        if (i0 < nm) store(k0, u0, s.hx.x, s.hy.x, s.hz.x, s.fx.x, s.fy.x, s.fz.x, s.sk.x);
+        if (i1 < nm) store(k1, u1, s.hx.y, s.hy.y, s.hz.y, s.fx.y, s.fy.y, s.fz.y, s.sk.y);
     }
     if (COUNT) {
         if (lane == 0) {
@@ -354,19 +382,18 @@ ff_walk_group(ff_walk_smem& sm, const int grp, const int lane,
 // Persistent launch: every warp fetches the next group from a device-wide counter (g->walk_next,
 // zeroed by the last cell-moment launch), so no SM idles while one block's slowest group finishes
 // and consecutive (spatially adjacent) groups run at the same time and share cells in L1/L2.
-template <bool COUNT>
+template <int W, bool COUNT, bool BUCKET>
 __global__ void __launch_bounds__(FF_WALK_WARPS * 32, FF_WALK_MINB)
 ff_k_walk(int n, int group_begin, int group_end, float theta, ff_globals* __restrict__ g, const float4* __restrict__ pos_s,
           const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
-          const int32_t* __restrict__ cell_first,
-          const int32_t* __restrict__ cell_end, const int4* __restrict__ cell_child,
+          const int4* __restrict__ cell_info, const int4* __restrict__ cell_child,
           const int32_t* __restrict__ leaf_count, const float4* __restrict__ centre,
           const float4* __restrict__ moment, float* __restrict__ H_out, float* __restrict__ F_out,
           unsigned long long* __restrict__ counters)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    ff_walk_smem& sm = reinterpret_cast<ff_walk_smem*>(smem_raw)[w];
+    ff_walk_smem<W>& sm = reinterpret_cast<ff_walk_smem<W>*>(smem_raw)[w];
     const int groups = group_end;                          // groups [group_begin, group_end) of the sorted order
     const int n_cells = g->n_cells;
     for (;;) {
@@ -374,38 +401,48 @@ ff_k_walk(int n, int group_begin, int group_end, float theta, ff_globals* __rest
         if (lane == 0) grp = group_begin + atomicAdd(&g->walk_next, 1);
         grp = __shfl_sync(FF_FULL, grp, 0);
         if (grp >= groups) break;
-        ff_walk_group<COUNT>(sm, grp, lane, n, theta, n_cells, pos_s, mom_s, perm, cell_first, cell_end, cell_child,
-                             leaf_count, centre, moment, H_out, F_out, counters);
+        ff_walk_group<W, COUNT, BUCKET>(sm, grp, lane, n, theta, n_cells, pos_s, mom_s, perm, cell_info, cell_child,
+                                        leaf_count, centre, moment, H_out, F_out, counters);
         __syncwarp();
     }
 }
 
+template <int W, bool COUNT, bool BUCKET>
+static int ff_launch_walk_t(ff_ctx* c, float* H_out, float* F_out, int group_begin, int group_end, int variant)
+{
+    const int n = (int)c->n;
+    const int groups = group_end - group_begin;
+    const size_t smem = sizeof(ff_walk_smem<W>) * FF_WALK_WARPS;
+    int& per_sm = c->occ_walk[variant];                    // per context: contexts may live on different devices
+    if (!per_sm) {
+        FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<W, COUNT, BUCKET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_walk<W, COUNT, BUCKET>, FF_WALK_WARPS * 32, smem));
+        if (per_sm < 1) return FF_ERR_CUDA;
+    }
+    const int blocks = min(c->num_sms * per_sm, (groups + FF_WALK_WARPS - 1) / FF_WALK_WARPS);
+    if (COUNT) FF_CUDA(c, cudaMemsetAsync(c->g->counters, 0, sizeof(c->g->counters), c->stream));
+    auto kernel = ff_k_walk<W, COUNT, BUCKET>;
+    FF_LAUNCH(c, kernel, blocks, FF_WALK_WARPS * 32, smem, n, group_begin, group_end, c->theta, c->g,
+              c->pos_s, c->mom_s, c->idx[0], c->cell_info, (const int4*)c->cell_child, c->leaf_count, c->cell_centre,
+              c->cell_moment, H_out, F_out, c->g->counters);
+    return FF_OK;
+}
+
 int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out, int group_begin, int group_end)
 {
-    int n = (int)c->n;
-    if (group_end < 0) group_end = (n + 31) / 32;
-    int groups = group_end - group_begin;
-    if (groups <= 0) return FF_OK;
-    size_t smem = sizeof(ff_walk_smem) * FF_WALK_WARPS;
-    int* per_sm = c->occ_walk;                             // per context: contexts may live on different devices
-    if (!per_sm[0]) {
-        FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], ff_k_walk<false>, FF_WALK_WARPS * 32, smem));
-        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], ff_k_walk<true>, FF_WALK_WARPS * 32, smem));
-        if (per_sm[0] < 1 || per_sm[1] < 1) return FF_ERR_CUDA;
+    const int n = (int)c->n, W = c->group;
+    if (group_end < 0) group_end = (n + W - 1) / W;
+    if (group_end - group_begin <= 0) return FF_OK;
+    const int cnt = c->count_enabled ? 1 : 0, bucket = c->nleaf > 1 ? 1 : 0;
+    const int variant = (W == 64 ? 4 : 0) + 2 * cnt + bucket;
+    switch (variant) {
+    case 0: return ff_launch_walk_t<32, false, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 1: return ff_launch_walk_t<32, false, true>(c, H_out, F_out, group_begin, group_end, variant);
+    case 2: return ff_launch_walk_t<32, true, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 3: return ff_launch_walk_t<32, true, true>(c, H_out, F_out, group_begin, group_end, variant);
+    case 4: return ff_launch_walk_t<64, false, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 5: return ff_launch_walk_t<64, false, true>(c, H_out, F_out, group_begin, group_end, variant);
+    case 6: return ff_launch_walk_t<64, true, false>(c, H_out, F_out, group_begin, group_end, variant);
+    default: return ff_launch_walk_t<64, true, true>(c, H_out, F_out, group_begin, group_end, variant);
     }
-    int cnt = c->count_enabled ? 1 : 0;
-    int blocks = min(c->num_sms * per_sm[cnt], (groups + FF_WALK_WARPS - 1) / FF_WALK_WARPS);
-    if (cnt) {
-        FF_CUDA(c, cudaMemsetAsync(c->g->counters, 0, sizeof(c->g->counters), c->stream));
-        FF_LAUNCH(c, ff_k_walk<true>, blocks, FF_WALK_WARPS * 32, smem, n, group_begin, group_end, c->theta, c->g, c->pos_s, c->mom_s,
-                  c->idx[0], c->cell_first, c->cell_end, (const int4*)c->cell_child,
-                  c->leaf_count, c->cell_centre, c->cell_moment, H_out, F_out, c->g->counters);
-    } else {
-        FF_LAUNCH(c, ff_k_walk<false>, blocks, FF_WALK_WARPS * 32, smem, n, group_begin, group_end, c->theta, c->g, c->pos_s, c->mom_s,
-                  c->idx[0], c->cell_first, c->cell_end, (const int4*)c->cell_child,
-                  c->leaf_count, c->cell_centre, c->cell_moment, H_out, F_out, c->g->counters);
-    }
-    return FF_OK;
 }

@@ -192,6 +192,36 @@ def eval_lists(lists, info, sp, sm, perm, scale=False):
     return (H, F, Q) if scale else (H, F)
 
 
+# ---- canonical form of the GPU tree (ff_tree_view) ----------------------------
+_FF_CHILD_EMPTY = -1
+_FF_CHILD_MULTI, _FF_CHILD_SLOT = 0x40000000, 0x3FFFFFFF
+
+
+def canonical_tree(tree: dict):
+    """Canonical topology [(first, level, prefix, count, is_leaf)] sorted by (first, level) from the dict of
+    FFContext.get_tree() (layout of ff_tree_view, include/ff.h): the internal cells plus the leaf children they point
+    to.  A test-side canonicaliser (reading Q7 of DESIGN.md: the GPU may number cells as it likes)."""
+    key = tree["key"].astype("int64")
+    n, m = tree["n"], tree["n_cells"]
+    out = []
+    if m == 0:
+        return [(0, 0, 0, n, 1)]
+    first, end, level, child = tree["cell_first"], tree["cell_end"], tree["cell_level"], tree["child"]
+    for i in range(m):
+        f, l = int(first[i]), int(level[i])
+        out.append((f, l, int(key[f] >> (3 * (10 - l))), int(end[i]) - f, 0))
+        for o in range(8):
+            e = int(child[i, o])
+            if e == _FF_CHILD_EMPTY or e >= 0:
+                continue
+            u = e & 0xFFFFFFFF
+            slot = u & _FF_CHILD_SLOT
+            cnt = int(tree["leaf_count"][slot]) if (u & _FF_CHILD_MULTI) else 1
+            out.append((slot, l + 1, int(key[slot] >> (3 * (10 - l - 1))), cnt, 1))
+    out.sort(key=lambda t: (t[0], t[1]))
+    return out
+
+
 # ---- error metric of DESIGN.md ("error metric", reading Q19) ------------------
 KAPPA = 8.0
 

@@ -3,7 +3,11 @@
 Tolerances (BASELINE.json north_star; error metric of DESIGN.md, reading Q19):
   Barnes-Hut vs oracle Barnes-Hut (same theta, same tree, same group rule) ... max_k e_k <= 1e-4
   direct vs oracle all-pairs ................................................. max_k e_k <= 1e-5
-  e_k = |x_k - ref_k|_2 / max(|ref_k|_2, Q_k / 8),  Q_k = sqrt(sum_j |term_kj|^2) from the oracle
+  Every case is gated on BOTH (helpers.check_hf)
+    e_k = |x_k - ref_k|_2 / max(|ref_k|_2, 1e-3 rms_k |ref|)       the survey's metric, no oracle scale
+    e_k = |x_k - ref_k|_2 / max(|ref_k|_2, Q_k / 8)                Q_k = sqrt(sum_j |term_kj|^2) from the oracle
+  except the head-to-tail chain inputs (config 4, the chain cases of the sweep), whose sums cancel by construction:
+  those use the second metric only.
   keys, permutation, root cube, cell topology, cell centres/moments .......... bit exact
 """
 import numpy as np
@@ -11,7 +15,7 @@ import pytest
 
 import ffgen
 import oracle
-from helpers import canonical_from_oracle, check_hf, rel_err
+from helpers import canonical_from_oracle, canonical_tree, check_hf, rel_err
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -32,8 +36,10 @@ def _dev(a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
 
 
-def _gpu_bh(ff, pos, mom, theta, nleaf=1, counters=True):
+def _gpu_bh(ff, pos, mom, theta, nleaf=1, counters=True, group=32):
     ctx = ff.FFContext(len(pos), theta, nleaf=nleaf, counters=counters)
+    if group != 32:
+        ctx.set_option(ff.FF_OPT_GROUP, group)
     p, m = _dev(pos), _dev(mom)
     ctx.build_tree(p)
     H, F = ctx.eval_bh(p, m)
@@ -48,7 +54,7 @@ def _check_tree(ff, ctx, otree, omom):
     assert np.array_equal(t["lo"], lo) and t["S"] == S
     assert np.array_equal(t["key"], okey)
     assert np.array_equal(t["perm"].astype(np.int64), operm)
-    assert ff.canonical_tree(t) == canonical_from_oracle(otree)
+    assert canonical_tree(t) == canonical_from_oracle(otree)
     # cell data, bit exact: match internal cells by (first, level)
     nd = otree.nodes()
     idx = {(int(f), int(l)): i for i, (f, l, leaf) in enumerate(zip(nd["first"], nd["level"], nd["is_leaf"])) if not leaf}
@@ -158,7 +164,64 @@ def test_random_sweep_of_theta_leaf_size_and_shape(ff, case):
     Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, theta, 32, nleaf=nleaf, scale=True)
     _check_tree(ff, ctx, otree, otree.moments(mom))
     assert ctx.counters() == cnt, (theta, nleaf, len(pos), shape)
-    check_hf(H, F, Ho, Fo, Q, TOL_BH)
+    # head-to-tail chains (shape 1): the neighbour forces cancel inside a chain, so the result carries the rounding
+    # error of terms far larger than itself; only there the survey's Q-free metric is not applied
+    check_hf(H, F, Ho, Fo, Q, TOL_BH, survey=shape != 1)
+
+
+@pytest.mark.parametrize("N,nleaf,theta,cfg", [(4096, 1, 0.5, 1), (1, 1, 0.5, 1), (33, 1, 0.5, 1), (64, 1, 0.5, 1),
+                                                (65, 1, 0.7, 1), (1000, 1, 0.3, 1), (4097, 4, 0.6, 1), (3000, 1, 0.5, 4),
+                                                (2500, 16, 1.0, 1)])
+def test_group_width_64(ff, N, nleaf, theta, cfg):
+    """FF_OPT_GROUP = 64 (reading Q2: the group rule with W = 64, one warp per group, two targets per lane): the same
+    checks as for W = 32 against the oracle walked with W = 64 -- identical interaction counters and H, F within 1e-4."""
+    c = ffgen.config(cfg, N=N, seed=N)
+    pos, mom = c["pos"], c["mom"]
+    ctx, H, F = _gpu_bh(ff, pos, mom, theta, nleaf=nleaf, group=64)
+    Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, theta, 64, nleaf=nleaf, scale=True)
+    _check_tree(ff, ctx, otree, otree.moments(mom))
+    assert ctx.counters() == cnt
+    if N > 1:
+        check_hf(H, F, Ho, Fo, Q, TOL_BH, survey=cfg != 4)
+    else:
+        assert np.all(H == 0) and np.all(F == 0)
+    # the group width is a property of the walk only: back to 32 on the same tree gives the W = 32 result
+    ctx.set_option(ff.FF_OPT_GROUP, 32)
+    p, m = _dev(pos), _dev(mom)
+    H32, F32 = ctx.eval_bh(p, m)
+    _, _, cnt32, _ = oracle.barnes_hut(pos, mom, theta, 32, nleaf=nleaf)
+    assert ctx.counters() == cnt32
+
+
+def test_skipping_one_output_leaves_the_other_unchanged(ff, cfg1):
+    """H_out / F_out = NULL (include/ff.h: "either may be NULL to skip it") on both evaluators: the output that is
+    asked for equals, bit for bit, the one of the call that asks for both, and nothing else is written."""
+    pos, mom = _dev(cfg1["pos"]), _dev(cfg1["mom"])
+    ctx = ff.FFContext(len(cfg1["pos"]), 0.5)
+    ctx.build_tree(pos)
+    H, F = ctx.eval_bh(pos, mom)
+    Hd, Fd = ctx.eval_direct(pos, mom)
+    Hn, Fn = ctx.eval_bh(pos, mom, want_F=False)
+    assert Fn is None and torch.equal(Hn, H)
+    Hn, Fn = ctx.eval_bh(pos, mom, want_H=False)
+    assert Hn is None and torch.equal(Fn, F)
+    L, h = ctx._L, ctx._h
+    guard = torch.full_like(H, 7.0)
+    out = torch.full_like(H, float("nan"))
+    n = len(cfg1["pos"])
+    ctx._check(L.ff_eval_direct(h, pos.data_ptr(), mom.data_ptr(), n, out.data_ptr(), None), "ff_eval_direct")
+    assert torch.equal(out, Hd)
+    ctx._check(L.ff_eval_direct(h, pos.data_ptr(), mom.data_ptr(), n, None, out.data_ptr()), "ff_eval_direct")
+    assert torch.equal(out, Fd)
+    ctx._check(L.ff_eval_bh(h, pos.data_ptr(), mom.data_ptr(), None, None), "ff_eval_bh")     # both skipped: legal
+    torch.cuda.synchronize()
+    assert bool((guard == 7.0).all())
+    # the small-N direct path (sources split over the grid + reduction) honours NULL as well
+    ps, ms = pos[:300].contiguous(), mom[:300].contiguous()
+    Hs, Fs = ctx.eval_direct(ps, ms)
+    out = torch.full_like(Hs, float("nan"))
+    ctx._check(L.ff_eval_direct(h, ps.data_ptr(), ms.data_ptr(), 300, None, out.data_ptr()), "ff_eval_direct")
+    assert torch.equal(out, Fs)
 
 
 def test_theta_zero_equals_all_pairs(ff):
@@ -316,9 +379,11 @@ def test_error_codes(ff):
         ctx.set_option(ff.FF_OPT_THETA, -1.0)
     with pytest.raises(ff.FFError):
         ctx.set_option(99, 1.0)
-    ctx.set_option(ff.FF_OPT_GROUP, 32)                                     # the one group width the GPU walk has
-    with pytest.raises(ff.FFError):
-        ctx.set_option(ff.FF_OPT_GROUP, 16)
+    ctx.set_option(ff.FF_OPT_GROUP, 32)                                     # the two group widths the GPU walk has
+    ctx.set_option(ff.FF_OPT_GROUP, 64)
+    for bad in (16, 1, 48, 128):
+        with pytest.raises(ff.FFError):
+            ctx.set_option(ff.FF_OPT_GROUP, bad)
 
 
 # ---------------------------------------------------------------- config 2 ----
@@ -351,7 +416,7 @@ def test_config2_theta_sweep(ff):
 
 
 # ------------------------------------------- full sizes, sampled oracle ----
-def _sampled_parity(ff, c, n_groups, seed=0):
+def _sampled_parity(ff, c, n_groups, seed=0, survey=True):
     pos, mom, theta = c["pos"], c["mom"], c["theta"]
     N = len(pos)
     ctx = ff.FFContext(N, theta)
@@ -374,7 +439,7 @@ def _sampled_parity(ff, c, n_groups, seed=0):
     Ho, Fo, _, Q = otree.eval(theta, 32, groups=groups, scale=True)
     rows = operm[(groups[:, None] * 32 + np.arange(32)[None, :]).ravel()]
     rows = rows[rows < N]
-    check_hf(H[rows], F[rows], Ho[rows], Fo[rows], Q[rows], TOL_BH)
+    check_hf(H[rows], F[rows], Ho[rows], Fo[rows], Q[rows], TOL_BH, survey=survey)
     assert np.isfinite(H).all() and np.isfinite(F).all()
     return ctx, H, F
 
@@ -386,7 +451,8 @@ def test_config3_one_million_sampled(ff):
 
 
 def test_config4_chains_sampled(ff):
-    _sampled_parity(ff, ffgen.config(4), 256)
+    # chains: the one full-size config whose sums cancel by construction -> term-scale metric only
+    _sampled_parity(ff, ffgen.config(4), 256, survey=False)
 
 
 def test_config5_sixteen_million_sampled(ff):
