@@ -49,12 +49,12 @@ ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n,
     const int k0 = blockIdx.x * FF_DIRECT_TARGETS + t, k1 = k0 + FF_DIRECT_THREADS;
     const size_t o0 = 3 * (size_t)min(k0, n - 1), o1 = 3 * (size_t)min(k1, n - 1);
     ff_target2 tg;
-    tg.px = make_float2(__ldg(pos + o0), __ldg(pos + o1));
-    tg.py = make_float2(__ldg(pos + o0 + 1), __ldg(pos + o1 + 1));
-    tg.pz = make_float2(__ldg(pos + o0 + 2), __ldg(pos + o1 + 2));
-    tg.ux = make_float2(__ldg(mom + o0), __ldg(mom + o1));
-    tg.uy = make_float2(__ldg(mom + o0 + 1), __ldg(mom + o1 + 1));
-    tg.uz = make_float2(__ldg(mom + o0 + 2), __ldg(mom + o1 + 2));
+    tg.px = ff_pin_pair(__ldg(pos + o0), __ldg(pos + o1));
+    tg.py = ff_pin_pair(__ldg(pos + o0 + 1), __ldg(pos + o1 + 1));
+    tg.pz = ff_pin_pair(__ldg(pos + o0 + 2), __ldg(pos + o1 + 2));
+    tg.ux = ff_pin_pair(__ldg(mom + o0), __ldg(mom + o1));
+    tg.uy = ff_pin_pair(__ldg(mom + o0 + 1), __ldg(mom + o1 + 1));
+    tg.uz = ff_pin_pair(__ldg(mom + o0 + 2), __ldg(mom + o1 + 2));
     double acc0[7] = { 0, 0, 0, 0, 0, 0, 0 }, acc1[7] = { 0, 0, 0, 0, 0, 0, 0 };
     const int n_tiles = (n + FF_DIRECT_THREADS - 1) / FF_DIRECT_THREADS;
     for (int tile = blockIdx.y; tile < n_tiles; tile += splits) {

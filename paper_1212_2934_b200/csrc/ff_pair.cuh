@@ -32,6 +32,18 @@ struct ff_target2 {
     float2 px, py, pz, ux, uy, uz;
 };
 
+// A register PAIR the compiler cannot rebuild from its two halves later on: without this ptxas keeps the two targets'
+// values in the registers they were loaded into and re-assembles the pairs with two MOVs per use inside the
+// evaluation loop (measured: +11 % instructions).  The volatile asm is opaque and cannot be duplicated.
+__device__ __forceinline__ float2 ff_pin_pair(float a, float b)
+{
+    unsigned long long v;
+    asm volatile("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(a), "f"(b));
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+
 // running sums of one lane for its two targets; f = fv + sk u_k (the u_k term of Eq. 12 is
 // accumulated as a scalar and applied once at the end).  The two parts of Eq. 11 go into ONE
 // accumulator: for aligned moments sum 3 rho (u.rho)/r^5 and sum u/r^3 are each far larger than

@@ -19,10 +19,10 @@
 // packed FP32 instructions of sm_100 (FFMA2 / FMUL2 / FADD2 through __ffma2_rn,
 // __fmul2_rn, __fadd2_rn).  Every lane holds TWO targets in the halves of its
 // register pairs and evaluates one source against both per instruction
-// (ff_pair.cuh).  W = 32: lanes l and l + 16 hold the same two targets (l, l + 16)
+// (ff_pair.cuh).  W = 32: lanes l and l + 16 hold the same two targets (2l, 2l + 1)
 // and split the sources of a batch between them (even / odd ring entries); the
 // two partial sums are added with one shuffle per accumulator at the end.
-// W = 64: lane l holds targets l and l + 32 and every lane evaluates every source.
+// W = 64: lane l holds targets 2l and 2l + 1 and every lane evaluates every source.
 //
 // Both phases produce exactly the interaction set of the oracle's recursive walk;
 // only the summation order differs.  fp32 arithmetic; the opening test uses
@@ -36,8 +36,10 @@ struct ff_walk_smem {
     int32_t stack[FF_WALK_STACK];
     float4 pendA[FF_WALK_PEND];        // ring entry e: x, y, z, mx
     float2 pendB[FF_WALK_PEND];        //               my, mz
-    float4 mem_xy[W / 2];              // group members in pairs for the opening test, pair m: x0,x1,y0,y1
-    float2 mem_z[W / 2];               //                                                   z0,z1
+    float4 mem_xy[W / 2];              // group members in pairs (pair m = members 2m, 2m + 1): x0,x1,y0,y1
+    float2 mem_z[W / 2];               //                                                        z0,z1
+    float4 mem_uxy[W / 2];             // their moments, same layout: ux0,ux1,uy0,uy1
+    float2 mem_uz[W / 2];              //                             uz0,uz1
     float4 probe_xy[FF_WALK_PROBE_PAIRS];   // probe members of the opening pre-filter, same pair layout
     float2 probe_z[FF_WALK_PROBE_PAIRS];
     float4 bb_lo, bb_hi;               // bounding box of the group's members (exact min / max)
@@ -62,41 +64,35 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
     const int nm = g1 - g0;
     const unsigned lt = (1u << lane) - 1u;
     const int half = (W == 32) ? (lane >> 4) : 0;          // W = 32: this lane takes the even (0) or odd (1) entries
-    const int i0 = (W == 32) ? (lane & 15) : lane;         // member indices of the lane's two targets
-    const int i1 = i0 + W / 2;
-
-    // own targets (members past a ragged end duplicate the last member; their results are dropped)
+    const int ti = (W == 32) ? (lane & 15) : lane;         // the lane's two targets are the ADJACENT members 2 ti, 2 ti + 1
+    const int i0 = 2 * ti, i1 = 2 * ti + 1;
     const int k0 = g0 + min(i0, nm - 1), k1 = g0 + min(i1, nm - 1);
-    const float4 p0 = __ldg(pos_s + k0), u0 = __ldg(mom_s + k0);
-    const float4 p1 = __ldg(pos_s + k1), u1 = __ldg(mom_s + k1);
-    ff_target2 tg;
-    tg.px = make_float2(p0.x, p1.x); tg.py = make_float2(p0.y, p1.y); tg.pz = make_float2(p0.z, p1.z);
-    tg.ux = make_float2(u0.x, u1.x); tg.uy = make_float2(u0.y, u1.y); tg.uz = make_float2(u0.z, u1.z);
-    ff_acc2 s;
-    ff_acc2_zero(s);
     unsigned long long c_cell = 0, c_part = 0, c_mac = 0, c_amb = 0;
 
-    {   // group members in pair layout for the opening test; the ring's first batch(es) = the members themselves
+    {   // Group members -> shared memory in pair layout (pair m = members 2m, 2m + 1) for the opening test and for the
+        // lanes' own target registers; the ring's first batch(es) = the members themselves.  Members past a ragged
+        // end duplicate the last member (their results are dropped).
         auto put_member = [&](int i, const float4& p, const float4& u) {
             float* mxy = reinterpret_cast<float*>(sm.mem_xy) + (i >> 1) * 4 + (i & 1);
             mxy[0] = p.x; mxy[2] = p.y;
             reinterpret_cast<float*>(sm.mem_z)[i] = p.z;
+            float* uxy = reinterpret_cast<float*>(sm.mem_uxy) + (i >> 1) * 4 + (i & 1);
+            uxy[0] = u.x; uxy[2] = u.y;
+            reinterpret_cast<float*>(sm.mem_uz)[i] = u.z;
             sm.pendA[i] = make_float4(p.x, p.y, p.z, u.x);
             sm.pendB[i] = make_float2(u.y, u.z);
         };
-        if (W == 32) {
-            put_member(lane, half ? p1 : p0, half ? u1 : u0);
-        } else {
-            put_member(i0, p0, u0);
-            put_member(i1, p1, u1);
-        }
+        const int ma = g0 + min(lane, nm - 1), mb = g0 + min(lane + 32, nm - 1);
+        const float4 pa = __ldg(pos_s + ma), ua = __ldg(mom_s + ma);
+        const float4 pb = (W == 64) ? __ldg(pos_s + mb) : pa, ub = (W == 64) ? __ldg(mom_s + mb) : ua;
+        put_member(lane, pa, ua);
+        if (W == 64) put_member(lane + 32, pb, ub);
         // pre-filter data: exact bounding box of the members and the probe members (the members that attain the x
-        // and y extremes of the box, chosen on a key that trades the low bits for the member index).  Members past
-        // a ragged end are copies of the last member, which is harmless.
-        const uint32_t ox = min(ff_f2ord(p0.x), ff_f2ord(p1.x)), oy = min(ff_f2ord(p0.y), ff_f2ord(p1.y)),
-                       oz = min(ff_f2ord(p0.z), ff_f2ord(p1.z));
-        const uint32_t Ox = max(ff_f2ord(p0.x), ff_f2ord(p1.x)), Oy = max(ff_f2ord(p0.y), ff_f2ord(p1.y)),
-                       Oz = max(ff_f2ord(p0.z), ff_f2ord(p1.z));
+        // and y extremes of the box, chosen on a key that trades the low bits for the member index)
+        const uint32_t ox = min(ff_f2ord(pa.x), ff_f2ord(pb.x)), oy = min(ff_f2ord(pa.y), ff_f2ord(pb.y)),
+                       oz = min(ff_f2ord(pa.z), ff_f2ord(pb.z));
+        const uint32_t Ox = max(ff_f2ord(pa.x), ff_f2ord(pb.x)), Oy = max(ff_f2ord(pa.y), ff_f2ord(pb.y)),
+                       Oz = max(ff_f2ord(pa.z), ff_f2ord(pb.z));
         const float lox = ff_ord2f(__reduce_min_sync(FF_FULL, ox)), hix = ff_ord2f(__reduce_max_sync(FF_FULL, Ox));
         const float loy = ff_ord2f(__reduce_min_sync(FF_FULL, oy)), hiy = ff_ord2f(__reduce_max_sync(FF_FULL, Oy));
         const float loz = ff_ord2f(__reduce_min_sync(FF_FULL, oz)), hiz = ff_ord2f(__reduce_max_sync(FF_FULL, Oz));
@@ -107,10 +103,10 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
         static_assert(FF_WALK_PROBE_PAIRS == 2, "four probe members: the x and y extremes");
         constexpr uint32_t IM = W - 1;                     // member index in the low bits of the key
         auto key = [&](float a, int i) { return (ff_f2ord(a) & ~IM) | (uint32_t)i; };
-        const int s0 = __reduce_min_sync(FF_FULL, min(key(p0.x, i0), key(p1.x, i1))) & IM;
-        const int s1 = __reduce_max_sync(FF_FULL, max(key(p0.x, i0), key(p1.x, i1))) & IM;
-        const int s2 = __reduce_min_sync(FF_FULL, min(key(p0.y, i0), key(p1.y, i1))) & IM;
-        const int s3 = __reduce_max_sync(FF_FULL, max(key(p0.y, i0), key(p1.y, i1))) & IM;
+        const int s0 = __reduce_min_sync(FF_FULL, min(key(pa.x, lane), key(pb.x, lane + W - 32))) & IM;
+        const int s1 = __reduce_max_sync(FF_FULL, max(key(pa.x, lane), key(pb.x, lane + W - 32))) & IM;
+        const int s2 = __reduce_min_sync(FF_FULL, min(key(pa.y, lane), key(pb.y, lane + W - 32))) & IM;
+        const int s3 = __reduce_max_sync(FF_FULL, max(key(pa.y, lane), key(pb.y, lane + W - 32))) & IM;
         __syncwarp();
         if (lane < 2 * FF_WALK_PROBE_PAIRS) {
             const int m = lane == 0 ? s0 : lane == 1 ? s1 : lane == 2 ? s2 : s3;
@@ -120,6 +116,17 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
             reinterpret_cast<float*>(sm.probe_z)[lane] = reinterpret_cast<const float*>(sm.mem_z)[m];
         }
     }
+    // own targets: read back from the pair layout with vector loads, so that every target value sits in an aligned
+    // register pair from the start (pairs assembled from separately loaded registers are rebuilt by ptxas with two
+    // MOVs per use inside the evaluation loop)
+    ff_target2 tg;
+    {
+        const float4 xy = sm.mem_xy[ti], uxy = sm.mem_uxy[ti];
+        tg.px = make_float2(xy.x, xy.y); tg.py = make_float2(xy.z, xy.w); tg.pz = sm.mem_z[ti];
+        tg.ux = make_float2(uxy.x, uxy.y); tg.uy = make_float2(uxy.z, uxy.w); tg.uz = sm.mem_uz[ti];
+    }
+    ff_acc2 s;
+    ff_acc2_zero(s);
     __syncwarp();
     // the group's own members: direct terms, self skipped by index (Alg. 1 line 5);
     // slots >= nm of a ragged last group hold copies of the last member and are masked the same way
@@ -355,19 +362,22 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
         FF_FOLD(s.hx); FF_FOLD(s.hy); FF_FOLD(s.hz); FF_FOLD(s.fx); FF_FOLD(s.fy); FF_FOLD(s.fz); FF_FOLD(s.sk);
 #undef FF_FOLD
     }
-    auto store = [&](int k, const float4& uk, float hx, float hy, float hz, float fvx, float fvy, float fvz, float sk) {
+    // (the moments are read back from the packed target registers: keeping the loaded float4 alive across the
+    // walk makes ptxas rebuild the register pairs with MOVs inside the evaluation loop)
+    auto store = [&](int k, float ux, float uy, float uz, float hx, float hy, float hz, float fvx, float fvy, float fvz,
+                     float sk) {
         const size_t o = (size_t)__ldg(perm + k) * 3;      // a7: back to caller order;  f = fv + sk u_k
         if (H_out) { H_out[o] = hx; H_out[o + 1] = hy; H_out[o + 2] = hz; }
-        if (F_out) { F_out[o] = fmaf(sk, uk.x, fvx); F_out[o + 1] = fmaf(sk, uk.y, fvy); F_out[o + 2] = fmaf(sk, uk.z, fvz); }
+        if (F_out) { F_out[o] = fmaf(sk, ux, fvx); F_out[o + 1] = fmaf(sk, uy, fvy); F_out[o + 2] = fmaf(sk, uz, fvz); }
     };
     if (W == 32) {
-        if (lane < nm) {
-            if (half) store(k1, u1, s.hx.y, s.hy.y, s.hz.y, s.fx.y, s.fy.y, s.fz.y, s.sk.y);
-            else store(k0, u0, s.hx.x, s.hy.x, s.hz.x, s.fx.x, s.fy.x, s.fz.x, s.sk.x);
+        if ((half ? i1 : i0) < nm) {
+            if (half) store(k1, tg.ux.y, tg.uy.y, tg.uz.y, s.hx.y, s.hy.y, s.hz.y, s.fx.y, s.fy.y, s.fz.y, s.sk.y);
+            else store(k0, tg.ux.x, tg.uy.x, tg.uz.x, s.hx.x, s.hy.x, s.hz.x, s.fx.x, s.fy.x, s.fz.x, s.sk.x);
         }
     } else {
-        if (i0 < nm) store(k0, u0, s.hx.x, s.hy.x, s.hz.x, s.fx.x, s.fy.x, s.fz.x, s.sk.x);
-        if (i1 < nm) store(k1, u1, s.hx.y, s.hy.y, s.hz.y, s.fx.y, s.fy.y, s.fz.y, s.sk.y);
+        if (i0 < nm) store(k0, tg.ux.x, tg.uy.x, tg.uz.x, s.hx.x, s.hy.x, s.hz.x, s.fx.x, s.fy.x, s.fz.x, s.sk.x);
+        if (i1 < nm) store(k1, tg.ux.y, tg.uy.y, tg.uz.y, s.hx.y, s.hy.y, s.hz.y, s.fx.y, s.fy.y, s.fz.y, s.sk.y);
     }
     if (COUNT) {
         if (lane == 0) {
