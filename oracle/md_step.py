@@ -35,16 +35,18 @@ from __future__ import annotations
 import numpy as np
 
 
-def lj_force(pos, eps: float, sigma: float, cutoff: float, chunk: int = 512):
-    """Eq. 13 summed over all j != k with |rho_kj| < cutoff.  pos [N][3] -> f^sr [N][3], fp64."""
+def lj_force(pos, eps: float, sigma: float, cutoff: float, chunk: int = 512, targets=None):
+    """Eq. 13 summed over all j != k with |rho_kj| < cutoff.  pos [N][3] -> f^sr [N][3], fp64.
+    targets: optional index array -> only those k are evaluated (still against ALL j) and row t belongs to targets[t]."""
     p = np.asarray(pos, dtype=np.float64)
     n = len(p)
-    f = np.zeros((n, 3))
-    for a in range(0, n, chunk):
-        rho = p[a:a + chunk, None, :] - p[None, :, :]             # rho_kj = rho_k - rho_j
+    tk = np.arange(n) if targets is None else np.asarray(targets, dtype=np.int64)
+    f = np.zeros((len(tk), 3))
+    for a in range(0, len(tk), chunk):
+        k = tk[a:a + chunk]
+        rho = p[k, None, :] - p[None, :, :]                       # rho_kj = rho_k - rho_j
         r2 = np.einsum("kja,kja->kj", rho, rho)
-        k = np.arange(a, min(n, a + chunk))
-        r2[k - a, k] = np.inf                                     # j != k, by index
+        r2[np.arange(len(k)), k] = np.inf                         # j != k, by index
         inside = r2 < cutoff * cutoff
         r2 = np.where(inside, r2, np.inf)
         sr6 = (sigma * sigma / r2) ** 3

@@ -32,14 +32,24 @@ def main():
     n_loc = common["N"] // world
     mine = full[rank * n_loc:(rank + 1) * n_loc].clone()
     gathered = bench.gather_particles(mine, world)
+    # the moments travel while the tree is built: begin / end pair around independent work
+    mom_full = torch.from_numpy(common["mom"])
+    pending = bench.gather_particles_begin(mom_full[rank * n_loc:(rank + 1) * n_loc].clone(), world)
+    busy = float(gathered.double().sum())                        # stands in for ff_build_tree(p_all)
+    mom_gathered = bench.gather_particles_end(pending)
     gb, ge = ff.shard_groups(common["N"], world, rank)
+    gb64, ge64 = ff.shard_groups(common["N"], world, rank, 64)
+    # the "strong" block of the JSON line from (fake) device times: one GPU 20 ms, sharded step 12.5 ms
+    strong = bench.strong_block(world, common["N"], 20.0, bench.max_over_ranks(12.5 - rank, world, torch.device("cpu")),
+                                0.5, 9.0, {"walk": 9.0})
     rec = {"rank": rank, "world": world, "local": local, "ms": ms, "rate": rate, "N": c["N"],
            "pos_sum": float(np.asarray(c["pos"], np.float64).sum()),
-           "gather_ok": bool(torch.equal(gathered, full)), "groups": [gb, ge]}
+           "gather_ok": bool(torch.equal(gathered, full)) and bool(torch.equal(mom_gathered, mom_full)) and busy == busy,
+           "groups": [gb, ge], "groups64": [gb64, ge64], "strong": strong}
     with open(os.path.join(out_dir, "rank%d.json" % rank), "w") as fh:
         json.dump(rec, fh)
     if rank == 0:
-        print(json.dumps({"value": rate, "n_gpus": world}))
+        print(json.dumps({"value": rate, "n_gpus": world, "scaling": "weak", "strong": strong}))
     dist.barrier()
     dist.destroy_process_group()
 

@@ -35,9 +35,18 @@ def test_two_rank_replicas_max_time_and_job_rate(tmp_path):
     # target sharding: the all-gather re-assembles the common ensemble on every rank, the group slices tile it
     assert all(x["gather_ok"] for x in recs)
     assert recs[0]["groups"] == [0, 32] and recs[1]["groups"] == [32, 64]
-    # exactly one JSON line, from rank 0
+    assert recs[0]["groups64"] == [0, 16] and recs[1]["groups64"] == [16, 32]
+    # exactly one JSON line, from rank 0, carrying both measurements: the weak-scaling headline and the "strong" block
     lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
-    assert len(lines) == 1 and json.loads(lines[0])["n_gpus"] == 2
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak"
+    st = d["strong"]
+    assert st["scaling"] == "strong" and st["n_gpus"] == 2 and st["N"] == 2048
+    assert st["ms_per_step"] == 12.5                                   # max over ranks of (12.5, 11.5)
+    assert abs(st["value"] - 2048 / 12.5e-3) < 1e-6                    # ONE ensemble: N, not world * N
+    assert abs(st["efficiency_vs_one_gpu"] - (20.0 / 2) / 12.5) < 1e-12
+    assert {"allgather_ms", "walk_ms_max_over_ranks", "one_gpu_ms_per_step", "phases_ms_rank0"} <= set(st)
 
 
 def test_reference_arm_runs_on_rank_zero_only():
