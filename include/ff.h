@@ -24,11 +24,12 @@
  *    and *_host functions synchronise that stream.
  *  - Return value: FF_OK (0) or a negative ff_status.  No exceptions cross the
  *    ABI.  One context per host thread; a context is bound to the device that
- *    was current at ff_create.
+ *    was current at ff_create: every call makes that device current while it runs
+ *    and restores the caller's device before it returns.
  *  - Undefined input (documented, not checked): non-finite values; two
  *    distinct particles at the same position (r = 0 gives inf/NaN exactly as
  *    in Eq. 11; the paper prevents it with the Lennard-Jones core);
- *    ff_eval_bh called with a `pos` other than the one the tree was built from.
+ *    ff_eval_bh called with a `pos` array whose CONTENT changed since ff_build_tree (the pointer is checked).
  *  - Units: the path is unit free (h ~ L^-3, f ~ L^-4).
  */
 #ifndef FF_H
@@ -48,7 +49,8 @@ typedef enum ff_status {
     FF_ERR_INVALID_ARG = -1,    /* NULL pointer, N <= 0, N > FF_MAX_N, theta < 0 or NaN, unknown option */
     FF_ERR_WORKSPACE = -2,      /* workspace NULL, too small or not 256-byte aligned */
     FF_ERR_NO_TREE = -3,        /* ff_eval_bh / ff_get_tree before ff_build_tree */
-    FF_ERR_CAPACITY = -4,       /* internal pool overflow (cannot happen with ff_workspace_bytes' sizing; kept for the ABI) */
+    FF_ERR_CAPACITY = -4,       /* internal pool overflow (cannot happen with ff_workspace_bytes' sizing; kept for the ABI).
+                                   Detected on the device, reported by the next ff_get_tree / ff_get_timings / ff_get_counters */
     FF_ERR_CUDA = -5            /* CUDA runtime / launch failure; text via ff_last_error */
 } ff_status;
 
@@ -114,7 +116,7 @@ int ff_build_tree(ff_ctx* ctx, const float* pos, int64_t n);
 
 /*
  * a5-a7: cell moments (Eq. 14) -> tree walk -> results in caller order.
- * pos must be the array the tree was built from; mom: device [n][3] fp32
+ * pos must be the array the tree was built from (another pointer is FF_ERR_INVALID_ARG); mom: device [n][3] fp32
  * (need not be unit length: Eq. 11-12 are bilinear in the moments).
  * H_out / F_out: device [n][3] fp32, either may be NULL to skip it.
  * H_out = sum_{j != k} h_kj only (no external field); F_out = f_k of Eq. 12,

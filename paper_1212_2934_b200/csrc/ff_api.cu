@@ -59,6 +59,22 @@ extern "C" size_t ff_workspace_bytes(int64_t N)
     return carve(nullptr, nullptr, N);
 }
 
+// everything ff_create made, in any state of completion
+static void ff_teardown(ff_ctx* c)
+{
+    for (int ph = 0; ph < FF_N_PHASES; ++ph)
+        for (int k = 0; k < 2; ++k) if (c->ev[ph][k]) cudaEventDestroy(c->ev[ph][k]);
+    for (int b = 0; b < 2; ++b) {
+        if (c->ev_pos[b]) cudaEventDestroy(c->ev_pos[b]);
+        if (c->ev_in[b]) cudaEventDestroy(c->ev_in[b]);
+        if (c->ev_done[b]) cudaEventDestroy(c->ev_done[b]);
+        if (c->ev_out[b]) cudaEventDestroy(c->ev_out[b]);
+    }
+    if (c->in_stream) cudaStreamDestroy(c->in_stream);
+    if (c->out_stream) cudaStreamDestroy(c->out_stream);
+    delete c;
+}
+
 extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, size_t workspace_bytes)
 {
     if (!out) return FF_ERR_INVALID_ARG;
@@ -85,7 +101,7 @@ extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, 
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_out[b], cudaEventDisableTiming);
     }
     if (e == cudaSuccess) e = cudaMemset(c->g, 0, sizeof(ff_globals));
-    if (e != cudaSuccess) { delete c; return FF_ERR_CUDA; }
+    if (e != cudaSuccess) { ff_teardown(c); return FF_ERR_CUDA; }
     *out = c;
     return FF_OK;
 }
@@ -93,20 +109,11 @@ extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, 
 extern "C" int ff_destroy(ff_ctx* c)
 {
     if (!c) return FF_ERR_INVALID_ARG;
+    ff_device_guard guard(c);
     cudaStreamSynchronize(c->stream);
-    for (int ph = 0; ph < FF_N_PHASES; ++ph)
-        for (int k = 0; k < 2; ++k) if (c->ev[ph][k]) cudaEventDestroy(c->ev[ph][k]);
     if (c->in_stream) cudaStreamSynchronize(c->in_stream);
     if (c->out_stream) cudaStreamSynchronize(c->out_stream);
-    for (int b = 0; b < 2; ++b) {
-        if (c->ev_pos[b]) cudaEventDestroy(c->ev_pos[b]);
-        if (c->ev_in[b]) cudaEventDestroy(c->ev_in[b]);
-        if (c->ev_done[b]) cudaEventDestroy(c->ev_done[b]);
-        if (c->ev_out[b]) cudaEventDestroy(c->ev_out[b]);
-    }
-    if (c->in_stream) cudaStreamDestroy(c->in_stream);
-    if (c->out_stream) cudaStreamDestroy(c->out_stream);
-    delete c;
+    ff_teardown(c);
     return FF_OK;
 }
 
@@ -142,6 +149,7 @@ extern "C" int ff_set_option(ff_ctx* c, int key, double value)
 
 extern "C" int ff_build_tree(ff_ctx* c, const float* pos, int64_t n)
 {
+    ff_device_guard guard(c);
     if (!c || !pos || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
     c->n = n;
     c->tree_built = 0;
@@ -157,6 +165,7 @@ extern "C" int ff_build_tree(ff_ctx* c, const float* pos, int64_t n)
     if ((rc = ff_launch_build(c)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_BUILD);
     c->tree_built = 1;
+    c->tree_pos = pos;
     return FF_OK;
 }
 
@@ -168,8 +177,10 @@ extern "C" int ff_eval_bh(ff_ctx* c, const float* pos, const float* mom, float* 
 extern "C" int ff_eval_bh_range(ff_ctx* c, const float* pos, const float* mom, float* H_out, float* F_out,
                                 int64_t group_begin, int64_t group_end)
 {
+    ff_device_guard guard(c);
     if (!c || !pos || !mom) return FF_ERR_INVALID_ARG;
     if (!c->tree_built) return FF_ERR_NO_TREE;
+    if (pos != c->tree_pos) return FF_ERR_INVALID_ARG;     // not the array the tree was built from
     const int64_t groups = (c->n + c->group - 1) / c->group;
     if (group_end < 0) group_end = groups;
     if (group_begin < 0 || group_begin > group_end || group_end > groups) return FF_ERR_INVALID_ARG;
@@ -186,6 +197,7 @@ extern "C" int ff_eval_bh_range(ff_ctx* c, const float* pos, const float* mom, f
 
 extern "C" int ff_eval_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n, float* H_out, float* F_out)
 {
+    ff_device_guard guard(c);
     if (!c || !pos || !mom || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
     ff_phase_begin(c, FF_PH_DIRECT);
     int rc = ff_launch_direct(c, pos, mom, n, H_out, F_out);
@@ -204,6 +216,7 @@ extern "C" int ff_eval_direct(ff_ctx* c, const float* pos, const float* mom, int
 // duplex), and inside one call the moment upload runs under the tree build.
 static int host_enqueue(ff_ctx* c, const float* pos_h, const float* mom_h, int64_t n, float* H_h, float* F_h, bool bh)
 {
+    ff_device_guard guard(c);
     if (!c || !pos_h || !mom_h || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
     const int b = (int)(c->host_seq & 1);
     const size_t bytes = (size_t)n * 12;
@@ -237,6 +250,7 @@ static int host_enqueue(ff_ctx* c, const float* pos_h, const float* mom_h, int64
 
 extern "C" int ff_host_sync(ff_ctx* c)
 {
+    ff_device_guard guard(c);
     if (!c) return FF_ERR_INVALID_ARG;
     FF_CUDA(c, cudaStreamSynchronize(c->in_stream));
     FF_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -264,6 +278,7 @@ extern "C" int ff_eval_direct_host(ff_ctx* c, const float* pos_h, const float* m
 extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n,
                        const ff_step_params* p, uint64_t step_index)
 {
+    ff_device_guard guard(c);
     if (!c || !pos || !vel || !mom || !angvel || !p || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
     if (!(p->dtau > 0.0f)) return FF_ERR_INVALID_ARG;
     int rc;
@@ -293,8 +308,17 @@ extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* ang
     return FF_OK;
 }
 
+// the sticky device-side error flag (FF_ERR_CAPACITY), read at a point where the stream is synchronised
+static int ff_device_error(ff_ctx* c)
+{
+    int32_t err = 0;
+    FF_CUDA(c, cudaMemcpy(&err, &c->g->error, sizeof(err), cudaMemcpyDeviceToHost));
+    return err;
+}
+
 extern "C" int ff_get_tree(ff_ctx* c, ff_tree_view* out)
 {
+    ff_device_guard guard(c);
     if (!c || !out) return FF_ERR_INVALID_ARG;
     if (!c->tree_built) return FF_ERR_NO_TREE;
     FF_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -314,6 +338,7 @@ extern "C" int ff_get_tree(ff_ctx* c, ff_tree_view* out)
 
 extern "C" int ff_get_timings(ff_ctx* c, float ms[FF_N_PHASES])
 {
+    ff_device_guard guard(c);
     if (!c || !ms) return FF_ERR_INVALID_ARG;
     FF_CUDA(c, cudaStreamSynchronize(c->stream));
     for (int ph = 0; ph < FF_N_PHASES; ++ph) {
@@ -323,11 +348,12 @@ extern "C" int ff_get_timings(ff_ctx* c, float ms[FF_N_PHASES])
             c->ev_valid[ph] = 0;
         }
     }
-    return FF_OK;
+    return ff_device_error(c);
 }
 
 extern "C" int ff_get_counters(ff_ctx* c, uint64_t* n_cell, uint64_t* n_particle, uint64_t* n_mac_tests)
 {
+    ff_device_guard guard(c);
     if (!c) return FF_ERR_INVALID_ARG;
     FF_CUDA(c, cudaStreamSynchronize(c->stream));
     unsigned long long v[3];
@@ -335,11 +361,12 @@ extern "C" int ff_get_counters(ff_ctx* c, uint64_t* n_cell, uint64_t* n_particle
     if (n_cell) *n_cell = v[0];
     if (n_particle) *n_particle = v[1];
     if (n_mac_tests) *n_mac_tests = v[2];
-    return FF_OK;
+    return ff_device_error(c);
 }
 
 extern "C" int ff_get_prefilter_count(ff_ctx* c, uint64_t* n_parked)
 {
+    ff_device_guard guard(c);
     if (!c || !n_parked) return FF_ERR_INVALID_ARG;
     FF_CUDA(c, cudaStreamSynchronize(c->stream));
     unsigned long long v;
@@ -357,12 +384,14 @@ extern "C" int ff_get_launch_count(ff_ctx* c, uint64_t* launches)
 
 extern "C" int ff_measure_fp32_peak(ff_ctx* c, int iters, double* tflops)
 {
+    ff_device_guard guard(c);
     if (!c || !tflops) return FF_ERR_INVALID_ARG;
     return ff_launch_probe(c, FF_PROBE_FFMA, iters, tflops);
 }
 
 extern "C" int ff_measure_probe(ff_ctx* c, int kind, int iters, double* tflops)
 {
+    ff_device_guard guard(c);
     if (!c || !tflops) return FF_ERR_INVALID_ARG;
     return ff_launch_probe(c, kind, iters, tflops);
 }

@@ -72,6 +72,7 @@ struct ff_ctx {
     int count_enabled;
     int timing_enabled;
     int tree_built;
+    const float* tree_pos;    // the pos array the current tree was built from (ff_eval_bh checks it is given the same one)
     int moments_valid;
     int device;
     int num_sms;
@@ -108,6 +109,19 @@ struct ff_ctx {
 
     cudaEvent_t ev[FF_N_PHASES][2];
     int ev_valid[FF_N_PHASES];
+};
+
+// Makes the context's device current for the duration of an ABI call and restores the caller's afterwards (a context
+// is bound to the device that was current at ff_create; the caller may have switched since).
+struct ff_device_guard {
+    int prev = -1, dev = -1;
+    explicit ff_device_guard(const ff_ctx* c)
+    {
+        if (!c) return;
+        dev = c->device;
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) cudaSetDevice(dev); else prev = -1;
+    }
+    ~ff_device_guard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
 // ---- error plumbing ------------------------------------------------------------

@@ -375,6 +375,14 @@ def test_error_codes(ff):
     with pytest.raises(ff.FFError) as e:
         ctx.build_tree(_dev(ffgen.uniform_points(101, 5.0, 0)))          # more particles than the context holds
     assert e.value.code == ff.FF_ERR_INVALID_ARG
+    # a tree is bound to the position array it was built from
+    ctx.build_tree(p)
+    other = p.clone()
+    with pytest.raises(ff.FFError) as e:
+        ctx.eval_bh(other, p)
+    assert e.value.code == ff.FF_ERR_INVALID_ARG
+    ctx.eval_bh(p, other)                                                   # the moments may be any array
+    assert ctx.counters()[0] >= 0 and isinstance(ctx.timings(), dict)       # also report the device-side error flag: none
     with pytest.raises(ff.FFError):
         ctx.set_option(ff.FF_OPT_THETA, -1.0)
     with pytest.raises(ff.FFError):

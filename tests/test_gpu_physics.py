@@ -79,6 +79,19 @@ def test_average_dipole_field_barnes_hut_vs_all_pairs():
     assert float(u[:, 2].mean()) > 0.5                       # the sample is magnetised, <h_z^dip> is not noise
     assert abs(hd) > 1e-3
     assert abs(hb - hd) <= 0.03 * abs(hd), (hb, hd)
+    # third leg: the fp64 oracle's all-pairs sum on the SAME configuration (the two GPU kernels share their pair
+    # arithmetic, so agreeing with each other proves less than agreeing with the oracle) -- <h_z> and every row
+    import oracle
+    xs, us = x.cpu().numpy(), u.cpu().numpy()
+    Ho, _, Qo = oracle.allpairs(xs, us, scale=True)
+    ho = float(Ho[:, 2].mean())
+    assert abs(hd - ho) <= 1e-5 * abs(ho), (hd, ho)
+    assert abs(hb - ho) <= 0.03 * abs(ho), (hb, ho)
+    e = np.linalg.norm(Hd.cpu().numpy() - Ho, axis=1) / np.maximum(np.linalg.norm(Ho, axis=1), Qo[:, 0] / 8.0)
+    assert e.max() <= 1e-5, e.max()
+    # ... and the oracle's Barnes-Hut <h_z> at the same theta and group width equals the GPU's
+    Hob, _, _, _ = oracle.barnes_hut(xs, us, 0.5, 32)
+    assert abs(hb - float(Hob[:, 2].mean())) <= 1e-5 * abs(ho)
     # the per-particle fields differ by the percent-level error of Eq. 14's lowest-order cell
     rel = float((Hb - Hd).double().norm() / Hd.double().norm())
     assert rel < 0.06

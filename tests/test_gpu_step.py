@@ -14,6 +14,10 @@ from oracle.md_step import lj_force, md_step, wall_force
 
 pytestmark = pytest.mark.gpu
 
+# north_star's Barnes-Hut tolerance, applied to the increments of the step (the increments are sums
+# of the Barnes-Hut force / torque, the pair force of Eq. 13 and the drag term, each carrying its own fp32 rounding)
+TOL_STEP = 1e-4
+
 
 @pytest.fixture(scope="module")
 def ff():
@@ -83,13 +87,13 @@ def _check_step(before, after, ref, aux, kw):
         scale = np.maximum(scale, np.linalg.norm(fsr, axis=1) / 8.0)
     scale = np.maximum(scale, np.linalg.norm(v0, axis=1) * ulp / dt * 4)       # fp32 rounding of v itself
     err = np.linalg.norm(acc_gpu - acc_ref, axis=1) / scale
-    assert err.max() <= 2e-4, err.max()
+    assert err.max() <= TOL_STEP, err.max()
     # angular-velocity increment / dtau = 5/2 (u x h - Gamma_r omega)
     t_gpu, t_ref = (w1 - w0) / dt, (wr - w0) / dt
     tscale = np.maximum(np.linalg.norm(t_ref, axis=1), 2.5 * Q[:, 0] / 8.0)
     tscale = np.maximum(tscale, np.linalg.norm(w0, axis=1) * ulp / dt * 4)
     terr = np.linalg.norm(t_gpu - t_ref, axis=1) / tscale
-    assert terr.max() <= 2e-4, terr.max()
+    assert terr.max() <= TOL_STEP, terr.max()
     # moments: unit length, and the same direction as the oracle's
     assert np.abs(np.linalg.norm(u1, axis=1) - 1.0).max() <= 4 * ulp
     assert np.abs(u1 - ur).max() <= 8 * ulp
