@@ -309,13 +309,14 @@ def _md_parity(ff, ctx, snap, kw, theta, seed):
     _, vr, _, wr = md_step(x0[rows], v0[rows], u0[rows], w0[rows], Ho[rows], Fo[rows], kw["dtau"], kw["gamma_d"],
                            kw["gamma_r"], kw["h_ext"], fsr)
     dt, ulp = kw["dtau"], 2.0 ** -24
+    # increments recovered from fp32 states carry the representation error 2^-24 |v1| / dtau of the stored result,
+    # whatever the forces are: subtracted before the relative gate (as in tests/test_gpu_step.py)
     acc_g, acc_r = (v1[rows] - v0[rows]) / dt, (vr - v0[rows]) / dt
-    scale = np.maximum(np.maximum(Qo[rows, 1], np.linalg.norm(fsr, axis=1)) / 8.0,
-                       np.linalg.norm(v0[rows], axis=1) * ulp / dt * 4)
-    e_acc = _rel_errs(acc_g, acc_r, scale)
+    scale = np.maximum(np.maximum(np.linalg.norm(acc_r, axis=1), Qo[rows, 1] / 8.0), np.linalg.norm(fsr, axis=1) / 8.0)
+    e_acc = np.maximum(np.linalg.norm(acc_g - acc_r, axis=1) - ulp * np.linalg.norm(v1[rows], axis=1) / dt, 0.0) / scale
     tq_g, tq_r = (w1[rows] - w0[rows]) / dt, (wr - w0[rows]) / dt
-    tscale = np.maximum(2.5 * Qo[rows, 0] / 8.0, np.linalg.norm(w0[rows], axis=1) * ulp / dt * 4)
-    e_tq = _rel_errs(tq_g, tq_r, tscale)
+    tscale = np.maximum(np.linalg.norm(tq_r, axis=1), 2.5 * Qo[rows, 0] / 8.0)
+    e_tq = np.maximum(np.linalg.norm(tq_g - tq_r, axis=1) - ulp * np.linalg.norm(w1[rows], axis=1) / dt, 0.0) / tscale
     return {"targets": int(len(rows)), "velocity_increment_max_err": float(e_acc.max()),
             "angular_velocity_increment_max_err": float(e_tq.max()),
             "max_lj_force": float(np.linalg.norm(fsr, axis=1).max())}
@@ -652,7 +653,7 @@ def run_ours(args):
             "phases_ms_last_step": last, "finite": bool(torch.isfinite(x).all() and torch.isfinite(u).all()),
             "params": {"dtau": kw["dtau"], "gamma_d": kw["gamma_d"], "gamma_r": kw["gamma_r"], "h_ext": list(kw["h_ext"]),
                        "lj": list(kw["lj"]), "noise": list(kw["noise"])},
-            "parity": {"by_step": md_par, "tolerance": 2e-4,
+            "parity": {"by_step": md_par, "tolerance": 1e-4,
                        "max_err": max(max(d["velocity_increment_max_err"], d["angular_velocity_increment_max_err"])
                                       for d in md_par.values()),
                        "how": "state of the running simulation before steps 0, 50, 99 -> one deterministic ff_step on a "

@@ -80,19 +80,24 @@ def _check_step(before, after, ref, aux, kw):
     ulp = 2.0 ** -24
     # positions: x + dtau v, one fp32 rounding of the result and of the product
     assert np.abs(x1 - xr).max() <= 4 * ulp * max(1.0, np.abs(xr).max())
-    # velocity increment / dtau = total force - drag: relative to the scale of the force terms
+    # velocity increment / dtau = total force - drag.  Two things are kept apart:
+    #  (1) the REPRESENTATION error of the fp32 state the increment is recovered from: v1 is stored with a relative
+    #      rounding of at most 2^-24 per component, i.e. an absolute 2^-24 |v1| / dtau in the increment, whatever the
+    #      forces are (it dominates for an isolated, slowly accelerating particle) -- subtracted before the gate;
+    #  (2) the error of the arithmetic of the step, gated at north_star's 1e-4 relative to the scale of the force
+    #      terms: max(|total|, Q_f / 8, |f_sr| / 8), as for the Barnes-Hut force itself.
     acc_gpu, acc_ref = (v1 - v0) / dt, (vr - v0) / dt
     scale = np.maximum(np.linalg.norm(acc_ref, axis=1), Q[:, 1] / 8.0)
     if fsr is not None:
         scale = np.maximum(scale, np.linalg.norm(fsr, axis=1) / 8.0)
-    scale = np.maximum(scale, np.linalg.norm(v0, axis=1) * ulp / dt * 4)       # fp32 rounding of v itself
-    err = np.linalg.norm(acc_gpu - acc_ref, axis=1) / scale
+    rep = ulp * np.linalg.norm(v1, axis=1) / dt
+    err = np.maximum(np.linalg.norm(acc_gpu - acc_ref, axis=1) - rep, 0.0) / scale
     assert err.max() <= TOL_STEP, err.max()
     # angular-velocity increment / dtau = 5/2 (u x h - Gamma_r omega)
     t_gpu, t_ref = (w1 - w0) / dt, (wr - w0) / dt
     tscale = np.maximum(np.linalg.norm(t_ref, axis=1), 2.5 * Q[:, 0] / 8.0)
-    tscale = np.maximum(tscale, np.linalg.norm(w0, axis=1) * ulp / dt * 4)
-    terr = np.linalg.norm(t_gpu - t_ref, axis=1) / tscale
+    trep = ulp * np.linalg.norm(w1, axis=1) / dt
+    terr = np.maximum(np.linalg.norm(t_gpu - t_ref, axis=1) - trep, 0.0) / tscale
     assert terr.max() <= TOL_STEP, terr.max()
     # moments: unit length, and the same direction as the oracle's
     assert np.abs(np.linalg.norm(u1, axis=1) - 1.0).max() <= 4 * ulp
