@@ -61,6 +61,12 @@ def _load():
         lib.ffo_tree_node_moments.argtypes = [vp] * 5
         lib.ffo_bh_eval.restype = i32
         lib.ffo_bh_eval.argtypes = [vp, f32, i32, i64, vp, vp, vp, vp, vp, i32]
+        lib.ffo_bh_eval_order.restype = i32
+        lib.ffo_bh_eval_order.argtypes = [vp, f32, i32, i32, i64, vp, vp, vp, vp, vp, i32]
+        lib.ffo_first_order.restype = None
+        lib.ffo_first_order.argtypes = [vp] * 6
+        lib.ffo_tree_node_dsym.restype = None
+        lib.ffo_tree_node_dsym.argtypes = [vp, vp]
         lib.ffo_bh_group_lists.restype = i32
         lib.ffo_bh_group_lists.argtypes = [vp, f32, i32, i64, vp, i64, vp, vp, i64, vp]
         _lib = lib
@@ -83,6 +89,16 @@ def pair(rk, uk, rj, uj):
     h = np.zeros(3)
     f = np.zeros(3)
     _load().ffo_pair(*[a.ctypes.data for a in args], h.ctypes.data, f.ctypes.data)
+    return h, f
+
+
+def first_order(rk, uk, rc, D):
+    """(dh, df): the first-order terms of a cell at rc with tensor D = sum_i (rho_i - rc) (x) u_i (3x3) acting on a
+    target at rk with moment uk (derivation in ff_oracle.c, O1b), fp64."""
+    args = [np.ascontiguousarray(x, dtype=np.float64) for x in (rk, uk, rc, np.asarray(D, np.float64).reshape(9))]
+    h = np.zeros(3)
+    f = np.zeros(3)
+    _load().ffo_first_order(*[a.ctypes.data for a in args], h.ctypes.data, f.ctypes.data)
     return h, f
 
 
@@ -153,12 +169,15 @@ class Tree:
         out = dict(sum_u=np.zeros((n, 3)), sum_p=np.zeros((n, 3)),
                    mu=np.zeros((n, 3), np.float32), cen=np.zeros((n, 3), np.float32))
         self._lib.ffo_tree_node_moments(self._t, *[out[k].ctypes.data for k in ("sum_u", "sum_p", "mu", "cen")])
+        out["dsym"] = np.zeros((n, 6), np.float32)          # first-order cell tensor, xx yy zz xy xz yz (8(f4))
+        self._lib.ffo_tree_node_dsym(self._t, out["dsym"].ctypes.data)
         return out
 
-    def eval(self, theta: float, W: int = 32, groups=None, nthreads: int = 0, scale: bool = False):
+    def eval(self, theta: float, W: int = 32, groups=None, nthreads: int = 0, scale: bool = False, order: int = 0):
         """Barnes-Hut H, F (fp64, caller order, (N,3)); rows outside `groups` are NaN.
         Returns (H, F, counters) with counters = (cell terms, particle terms, opening tests);
-        scale=True appends Q (N, 2), the per-target root-sum-square of the term magnitudes."""
+        scale=True appends Q (N, 2), the per-target root-sum-square of the term magnitudes.
+        order=1 adds the first-order term of every accepted cell; 0 is the paper's cell."""
         assert self._mom is not None, "call moments(mom) first"
         H = np.full((self.N, 3), np.nan)
         F = np.full((self.N, 3), np.nan)
@@ -169,8 +188,8 @@ class Tree:
             groups = np.ascontiguousarray(groups, dtype=np.int64)
             ng, gp = groups.shape[0], groups.ctypes.data
         Q = np.full((self.N, 2), np.nan) if scale else None
-        rc = self._lib.ffo_bh_eval(self._t, float(theta), int(W), ng, gp, H.ctypes.data, F.ctypes.data,
-                                   Q.ctypes.data if scale else None, cnt.ctypes.data, nthreads)
+        rc = self._lib.ffo_bh_eval_order(self._t, float(theta), int(W), int(order), ng, gp, H.ctypes.data, F.ctypes.data,
+                                         Q.ctypes.data if scale else None, cnt.ctypes.data, nthreads)
         if rc != 0:
             raise RuntimeError("ffo_bh_eval failed")
         cnt = tuple(int(c) for c in cnt)
@@ -191,9 +210,9 @@ class Tree:
 
 
 def barnes_hut(pos, mom, theta: float, W: int = 32, nleaf: int = 1, groups=None, nthreads: int = 0,
-               scale: bool = False):
+               scale: bool = False, order: int = 0):
     """Convenience: build, moments, evaluate.  Returns (H, F, counters, tree) [+ (Q,) if scale]."""
     t = Tree(pos, nleaf)
     t.moments(mom)
-    out = t.eval(theta, W, groups, nthreads, scale)
+    out = t.eval(theta, W, groups, nthreads, scale, order)
     return (out[0], out[1], out[2], t) + ((out[3],) if scale else ())

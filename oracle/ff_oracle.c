@@ -22,6 +22,11 @@
  *   ffo_bh_eval ......... theta = 0 == all-pairs, N <= N_leaf == all-pairs,
  *                         independently written recursive list builder on
  *                         N <= 64, far-cluster limit, (28 pi/3) theta^-3 count
+ *   Q output (scale) .... independent numpy sum of squared terms (all-pairs and the list builder's lists),
+ *                         exact-rational closed form on the straight chain (tests/test_oracle_scale.py)
+ *   first-order cell term (O1b, not in the paper): central differences of Eq. 11-12 in the source
+ *                         position, error order (s/d)^2 on the far cluster and on a two-particle cell, theta = 0
+ *                         unchanged, D against numpy (tests/test_oracle_first_order.py)
  *   BH-vs-all-pairs error SIZE: parity unpinned by the paper (PAPER.md:233,
  *                         239 only say "almost identical"); reported, not gated.
  *
@@ -81,6 +86,61 @@ void ffo_pair(const double rk[3], const double uk[3], const double rj[3], const 
     h[0] = h[1] = h[2] = 0.0;
     f[0] = f[1] = f[2] = 0.0;
     pair_accumulate(rk, uk, rj, uj, h, f, NULL);
+}
+
+/* ----------------------------------------------------------------- O1b --
+ * First-order correction of a cell's pseudo-particle (NOT in the paper, whose cell is the
+ * lowest-order term only).  A cell's exact field at a target is sum_i T(rho_k - rho_i) u_i with
+ * the dipole tensor of Eq. 11, T_ab(r) = (3 r_a r_b - delta_ab r^2) / r^5.  Expanding each rho_i = rho' + d_i about
+ * the cell centre rho' of Eq. 14, with R = rho_k - rho':
+ *     h_a = T_ab(R) u'_b  -  S_abc(R) D_cb  +  O(d^2),        D_cb = sum_i d_ic u_ib,
+ *     S_abc = dT_ab/dr_c = 3 (delta_ab r_c + delta_ac r_b + delta_bc r_a) / r^5 - 15 r_a r_b r_c / r^7
+ * (the same S that gives Eq. 12: f_a = S_abc u_kb u_jc).  The force on the target dipole is f_a = u_kb d(h_b)/dr_a:
+ *     f_a = S_abc u_kb u'_c  -  U_abcd u_kb D_cd,
+ *     U_abcd = dS_bcd/dr_a = 3 (d_ab d_cd + d_ac d_bd + d_ad d_bc) / r^5
+ *              - 15 (d_ab r_c r_d + d_ac r_b r_d + d_ad r_b r_c + d_bc r_a r_d + d_bd r_a r_c + d_cd r_a r_b) / r^7
+ *              + 105 r_a r_b r_c r_d / r^9                                         (d_xy = Kronecker delta).
+ * Written out as plain loops over the tensor components.  D is the full 3x3 tensor here; the tree stores its
+ * symmetric part only (S and U are symmetric in the contracted index pairs, so the antisymmetric part drops out).
+ * The correction terms are ADDED to h, f.
+ */
+static double kd(int a, int b) { return a == b ? 1.0 : 0.0; }
+
+static void first_order_accumulate(const double rk[3], const double uk[3], const double rc[3], const double D[3][3],
+                                   double h[3], double f[3], double* q /* NULL or [2] */)
+{
+    double r[3] = { rk[0] - rc[0], rk[1] - rc[1], rk[2] - rc[2] };
+    double r2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+    double rr = sqrt(r2), r5 = r2 * r2 * rr, r7 = r5 * r2, r9 = r7 * r2;
+    double th2 = 0.0, tf2 = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        double dh = 0.0, df = 0.0;
+        for (int b = 0; b < 3; ++b)
+            for (int c = 0; c < 3; ++c) {
+                double S = 3.0 * (kd(a, b) * r[c] + kd(a, c) * r[b] + kd(b, c) * r[a]) / r5 - 15.0 * r[a] * r[b] * r[c] / r7;
+                dh -= S * D[c][b];
+                for (int d = 0; d < 3; ++d) {
+                    double U = 3.0 * (kd(a, b) * kd(c, d) + kd(a, c) * kd(b, d) + kd(a, d) * kd(b, c)) / r5
+                               - 15.0 * (kd(a, b) * r[c] * r[d] + kd(a, c) * r[b] * r[d] + kd(a, d) * r[b] * r[c]
+                                         + kd(b, c) * r[a] * r[d] + kd(b, d) * r[a] * r[c] + kd(c, d) * r[a] * r[b]) / r7
+                               + 105.0 * r[a] * r[b] * r[c] * r[d] / r9;
+                    df -= U * uk[b] * D[c][d];
+                }
+            }
+        h[a] += dh; f[a] += df;
+        th2 += dh * dh; tf2 += df * df;
+    }
+    if (q) { q[0] += th2; q[1] += tf2; }
+}
+
+/* public entry for the pins: h, f are OVERWRITTEN with the first-order terms of a cell at rc with tensor D (row major) */
+void ffo_first_order(const double rk[3], const double uk[3], const double rc[3], const double D9[9], double h[3], double f[3])
+{
+    double D[3][3];
+    for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) D[a][b] = D9[3 * a + b];
+    h[0] = h[1] = h[2] = 0.0;
+    f[0] = f[1] = f[2] = 0.0;
+    first_order_accumulate(rk, uk, rc, D, h, f, NULL);
 }
 
 static void widen3(const float* src, int64_t i, double out[3])
@@ -143,6 +203,8 @@ typedef struct {
     int64_t child[8];         /* node index per octant, -1 = empty sub-cell */
     double sum_u[3], sum_p[3];/* O4: fp64 sums in the fixed recursion order */
     float cen[3], mu[3];      /* O4: rho' and u' rounded once to fp32 */
+    double sum_pu[6];         /* O4b: fp64 sums of the symmetrised products rho_i (x) u_i, order xx yy zz xy xz yz */
+    float dsym[6];            /* O4b: first-order cell tensor D (symmetric part), rounded once to fp32 */
 } ffo_node;
 
 typedef struct ffo_tree {
@@ -313,20 +375,36 @@ void ffo_tree_nodes(const ffo_tree* t, int64_t* first, int64_t* count, int32_t* 
  * internal: children in octant order 0..7, ((c0 + c1) + c2) + ... -- then one
  * fp64 divide and ONE rounding to fp32.  The fp32 values are the node data.
  */
+/* symmetrised products of one particle, order xx yy zz xy xz yz: rho_a u_a and (rho_a u_b + rho_b u_a) / 2.
+ * Products of two fp32 values are exact in fp64; the sum of two of them is rounded once; the halving is exact. */
+static void sym_products(const float* p, const float* u, double out[6])
+{
+    double px = p[0], py = p[1], pz = p[2], ux = u[0], uy = u[1], uz = u[2];
+    out[0] = px * ux; out[1] = py * uy; out[2] = pz * uz;
+    out[3] = (px * uy + py * ux) * 0.5;
+    out[4] = (px * uz + pz * ux) * 0.5;
+    out[5] = (py * uz + pz * uy) * 0.5;
+}
+
 static void moments_cell(ffo_tree* t, int64_t id)
 {
     ffo_node* n = &t->node[id];
-    double su[3], sp[3];
+    double su[3], sp[3], spu[6];
     if (n->is_leaf) {
         for (int a = 0; a < 3; ++a) {
             su[a] = (double)t->smom[3 * n->first + a];
             sp[a] = (double)t->spos[3 * n->first + a];
         }
-        for (int64_t s = n->first + 1; s < n->first + n->count; ++s)
+        sym_products(t->spos + 3 * n->first, t->smom + 3 * n->first, spu);
+        for (int64_t s = n->first + 1; s < n->first + n->count; ++s) {
+            double pu[6];
+            sym_products(t->spos + 3 * s, t->smom + 3 * s, pu);
             for (int a = 0; a < 3; ++a) {
                 su[a] += (double)t->smom[3 * s + a];
                 sp[a] += (double)t->spos[3 * s + a];
             }
+            for (int a = 0; a < 6; ++a) spu[a] += pu[a];
+        }
     } else {
         int started = 0;
         for (int o = 0; o < 8; ++o) {
@@ -339,13 +417,27 @@ static void moments_cell(ffo_tree* t, int64_t id)
                 if (!started) { su[a] = cn->sum_u[a]; sp[a] = cn->sum_p[a]; }
                 else { su[a] += cn->sum_u[a]; sp[a] += cn->sum_p[a]; }
             }
+            for (int a = 0; a < 6; ++a) {
+                if (!started) spu[a] = cn->sum_pu[a];
+                else spu[a] += cn->sum_pu[a];
+            }
             started = 1;
         }
     }
+    double cen[3];
     for (int a = 0; a < 3; ++a) {
         n->sum_u[a] = su[a]; n->sum_p[a] = sp[a];
         n->mu[a] = (float)su[a];
-        n->cen[a] = (float)(sp[a] / (double)n->count);
+        cen[a] = sp[a] / (double)n->count;
+        n->cen[a] = (float)cen[a];
+    }
+    /* O4b: D = sum_i (rho_i - rho') (x) u_i, symmetric part = sum of the symmetrised products minus the symmetrised
+     * rho' (x) u' (fp64 rho' before its rounding, fp64 u'), each operation rounded once in fp64, the result once to fp32 */
+    static const int ia[6] = { 0, 1, 2, 0, 0, 1 }, ib[6] = { 0, 1, 2, 1, 2, 2 };
+    for (int c = 0; c < 6; ++c) {
+        n->sum_pu[c] = spu[c];
+        double cu = c < 3 ? cen[ia[c]] * su[ib[c]] : (cen[ia[c]] * su[ib[c]] + cen[ib[c]] * su[ia[c]]) * 0.5;
+        n->dsym[c] = (float)(spu[c] - cu);
     }
 }
 
@@ -359,6 +451,13 @@ int ffo_tree_moments(ffo_tree* t, const float* mom)
     moments_cell(t, 0);
     t->has_moments = 1;
     return 0;
+}
+
+/* O4b node data: dsym [n][6] fp32 in the order xx yy zz xy xz yz */
+void ffo_tree_node_dsym(const ffo_tree* t, float* dsym)
+{
+    for (int64_t i = 0; i < t->n_nodes; ++i)
+        for (int c = 0; c < 6; ++c) dsym[6 * i + c] = t->node[i].dsym[c];
 }
 
 void ffo_tree_node_moments(const ffo_tree* t, double* sum_u, double* sum_p, float* mu, float* cen)
@@ -395,6 +494,7 @@ void ffo_tree_node_moments(const ffo_tree* t, double* sum_u, double* sum_p, floa
 typedef struct {
     const ffo_tree* t;
     float th2;
+    int order;                /* 0 = the paper's cell (Eq. 14); 1 = plus the first-order term O1b */
     int64_t g0, g1;           /* group = sorted slots [g0, g1) */
     double* h; double* f;     /* [g1-g0][3] accumulators (NULL when only listing) */
     double* q;                /* [g1-g0][2] squared term magnitudes (error-metric scale) */
@@ -453,7 +553,22 @@ static void visit(walk_ctx* w, int64_t id)
                 for (int64_t k = w->g0; k < w->g1; ++k) {
                     double rk[3], uk[3];
                     widen3(t->spos, k, rk); widen3(t->smom, k, uk);
-                    pair_accumulate(rk, uk, rj, uj, w->h + 3 * (k - w->g0), w->f + 3 * (k - w->g0), w->q + 2 * (k - w->g0));
+                    if (!w->order) {
+                        pair_accumulate(rk, uk, rj, uj, w->h + 3 * (k - w->g0), w->f + 3 * (k - w->g0), w->q + 2 * (k - w->g0));
+                    } else {
+                        /* the cell's term = pseudo-particle + first-order correction; its magnitude enters q as ONE term */
+                        double th[3] = { 0, 0, 0 }, tf[3] = { 0, 0, 0 };
+                        double D[3][3] = { { n->dsym[0], n->dsym[3], n->dsym[4] },
+                                           { n->dsym[3], n->dsym[1], n->dsym[5] },
+                                           { n->dsym[4], n->dsym[5], n->dsym[2] } };
+                        pair_accumulate(rk, uk, rj, uj, th, tf, NULL);
+                        first_order_accumulate(rk, uk, rj, D, th, tf, NULL);
+                        double* hh = w->h + 3 * (k - w->g0); double* ff = w->f + 3 * (k - w->g0); double* qq = w->q + 2 * (k - w->g0);
+                        for (int a = 0; a < 3; ++a) {
+                            hh[a] += th[a]; ff[a] += tf[a];
+                            qq[0] += th[a] * th[a]; qq[1] += tf[a] * tf[a];
+                        }
+                    }
                 }
                 w->n_cell += (uint64_t)(w->g1 - w->g0);
             }
@@ -472,10 +587,10 @@ static void visit(walk_ctx* w, int64_t id)
  * particle terms summed over targets (self excluded), [2] = opening tests
  * (group, internal node not holding a member) evaluated.
  */
-int ffo_bh_eval(const ffo_tree* t, float theta, int W, int64_t ng, const int64_t* groups,
-                double* H, double* F, double* Q /* NULL or [N][2], caller order */, uint64_t counters[3], int nthreads)
+int ffo_bh_eval_order(const ffo_tree* t, float theta, int W, int order, int64_t ng, const int64_t* groups,
+                      double* H, double* F, double* Q /* NULL or [N][2], caller order */, uint64_t counters[3], int nthreads)
 {
-    if (!t || !t->has_moments || W < 1 || !(theta >= 0.0f) || !H || !F) return -1;
+    if (!t || !t->has_moments || W < 1 || !(theta >= 0.0f) || !H || !F || order < 0 || order > 1) return -1;
     int64_t n_groups = (t->N + W - 1) / W;
     if (!groups) ng = n_groups;
     float th2 = theta * theta;
@@ -488,7 +603,7 @@ int ffo_bh_eval(const ffo_tree* t, float theta, int W, int64_t ng, const int64_t
         if (g < 0 || g >= n_groups) continue;
         walk_ctx w;
         memset(&w, 0, sizeof(w));
-        w.t = t; w.th2 = th2;
+        w.t = t; w.th2 = th2; w.order = order;
         w.g0 = g * W; w.g1 = w.g0 + W < t->N ? w.g0 + W : t->N;
         int64_t m = w.g1 - w.g0;
         double* acc = (double*)calloc((size_t)m * 8, sizeof(double));
@@ -509,6 +624,13 @@ int ffo_bh_eval(const ffo_tree* t, float theta, int W, int64_t ng, const int64_t
     }
     if (counters) { counters[0] = c0; counters[1] = c1; counters[2] = c2; }
     return 0;
+}
+
+/* the paper's cell (order 0) */
+int ffo_bh_eval(const ffo_tree* t, float theta, int W, int64_t ng, const int64_t* groups,
+                double* H, double* F, double* Q, uint64_t counters[3], int nthreads)
+{
+    return ffo_bh_eval_order(t, theta, W, 0, ng, groups, H, F, Q, counters, nthreads);
 }
 
 /*

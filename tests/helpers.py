@@ -71,6 +71,27 @@ def allpairs_numpy(pos, mom):
     return H, F
 
 
+# ---- first-order cell term, contracted closed form -------------
+def first_order_terms(rk, uk, rc, D):
+    """First-order terms (dh, df) of a cell at rc with tensor D = sum_i (rho_i - rc) (x) u_i acting on a target at rk
+    with moment uk, from the CONTRACTED form of the Taylor expansion of Eq. 11-12 about the cell centre
+    (with R = rk - rc, Ds = (D + D^T) / 2, t = tr D, b = uk.R, q = R.Ds.R):
+        dh = -{ 3 [2 Ds R + t R] / R^5 - 15 R q / R^7 }
+        df = -{ 3 [2 Ds uk + t uk] / R^5 - 15 [R (2 uk.Ds.R + t b) + uk q + 2 b Ds R] / R^7 + 105 R b q / R^9 }
+    Written independently of the oracle, which loops over the components of the rank-3 / rank-4 derivative tensors."""
+    R = np.asarray(rk, float) - np.asarray(rc, float)
+    u = np.asarray(uk, float)
+    D = np.asarray(D, float).reshape(3, 3)
+    Ds = 0.5 * (D + D.T)
+    t = np.trace(D)
+    r = np.sqrt(R @ R)
+    DR, Du = Ds @ R, Ds @ u
+    q, b, uDR = R @ DR, u @ R, u @ DR
+    dh = -(3 * (2 * DR + t * R) / r**5 - 15 * R * q / r**7)
+    df = -(3 * (2 * Du + t * u) / r**5 - 15 * (R * (2 * uDR + t * b) + u * q + 2 * b * DR) / r**7 + 105 * R * b * q / r**9)
+    return dh, df
+
+
 # ---- tree by brute-force prefix grouping (reading O3) -----------------------
 def morton_keys_numpy(pos):
     """30-bit keys, fp32 arithmetic in the order inv=fl(1024/S); q=floor(fl(fl(p-lo)*inv))."""
