@@ -63,6 +63,10 @@ enum {
     FF_OPT_NLEAF = 2,     /* leaf capacity N_leaf >= 1; 1 = the paper's tree. Invalidates the tree. */
     FF_OPT_COUNTERS = 3,  /* != 0: the walk also counts interactions (slower); read with ff_get_counters */
     FF_OPT_TIMING = 4,    /* != 0: record CUDA events around each phase; read with ff_get_timings */
+    FF_OPT_CELL_ORDER = 6, /* 0 (default): a cell acts as the paper's pseudo-particle, Eq. 14.  1: plus the
+                             first-order term of the expansion of Eq. 11-12 about the cell centre, with the cell tensor
+                             D = sum_i (rho_i - rho') (x) u_i (not in the paper).
+                             Same interaction lists; W = 32 only */
     FF_OPT_GROUP = 5      /* targets per walk group W (reading Q2): 32 (default) or 64, one warp per group with
                              two targets per lane; any other value is FF_ERR_INVALID_ARG (the oracle takes any W) */
 };
@@ -241,6 +245,8 @@ typedef struct ff_tree_view {
     const int32_t* leaf_count; /* [n] defined at the first slot of multi-particle leaves */
     const float* cell_centre;  /* [n_cells][4] rho'.xyz (fp32), fl(s_l^2); valid after ff_eval_bh */
     const float* cell_moment;  /* [n_cells][4] u'.xyz (fp32), N' as float; valid after ff_eval_bh */
+    const float* cell_quad;    /* [n_cells][8] FF_OPT_CELL_ORDER = 1 only (else NULL): symmetric part of the cell tensor D,
+                                  xx yy zz xy xz yz 0 0 (fp32); valid after ff_eval_bh */
 } ff_tree_view;
 
 int ff_get_tree(ff_ctx* ctx, ff_tree_view* out);

@@ -22,7 +22,7 @@ _lib = None
 
 FF_OK = 0
 FF_ERR_INVALID_ARG, FF_ERR_WORKSPACE, FF_ERR_NO_TREE, FF_ERR_CAPACITY, FF_ERR_CUDA = -1, -2, -3, -4, -5
-FF_OPT_THETA, FF_OPT_NLEAF, FF_OPT_COUNTERS, FF_OPT_TIMING, FF_OPT_GROUP = 1, 2, 3, 4, 5
+FF_OPT_THETA, FF_OPT_NLEAF, FF_OPT_COUNTERS, FF_OPT_TIMING, FF_OPT_GROUP, FF_OPT_CELL_ORDER = 1, 2, 3, 4, 5, 6
 FF_N_PHASES = 7
 PHASES = ("bbox_keys", "sort", "build", "moments", "walk", "direct", "step")
 FF_PROBE_FFMA, FF_PROBE_FFMA2_PAIRS, FF_PROBE_FFMA2_REUSE, FF_PROBE_FFMA2_SCALAR, FF_PROBE_EVAL = 0, 1, 2, 3, 4
@@ -53,7 +53,7 @@ class ff_tree_view(ctypes.Structure):
                 ("key", ctypes.c_void_p), ("perm", ctypes.c_void_p), ("pos_sorted", ctypes.c_void_p),
                 ("mom_sorted", ctypes.c_void_p), ("cell_first", ctypes.c_void_p), ("cell_end", ctypes.c_void_p),
                 ("cell_level", ctypes.c_void_p), ("child", ctypes.c_void_p), ("leaf_count", ctypes.c_void_p),
-                ("cell_centre", ctypes.c_void_p), ("cell_moment", ctypes.c_void_p)]
+                ("cell_centre", ctypes.c_void_p), ("cell_moment", ctypes.c_void_p), ("cell_quad", ctypes.c_void_p)]
 
 
 def shard_groups(n: int, world: int, rank: int, group: int = 32):
@@ -291,7 +291,11 @@ class FFContext:
             return self.workspace[off:off + nbytes].view(dtype).cpu().numpy()
 
         n, m = int(v.n), int(v.n_cells)
+        extra = {}
+        if v.cell_quad:
+            extra["cell_quad"] = arr(v.cell_quad, 8 * m, torch.float32).reshape(m, 8)
         return dict(
+            **extra,
             n=n, n_cells=m, nleaf=int(v.nleaf), lo=np.array(list(v.lo), np.float32), S=np.float32(v.S),
             key=arr(v.key, n, torch.int32).view(np.uint32), perm=arr(v.perm, n, torch.int32).view(np.uint32),
             pos_sorted=arr(v.pos_sorted, 4 * n, torch.float32).reshape(n, 4),

@@ -40,6 +40,8 @@ static size_t carve(ff_ctx* c, char* base, int64_t N)
     p = take(cap * 16);                           if (c) c->cell_centre = (float4*)p;
     p = take(cap * 16);                           if (c) c->cell_moment = (float4*)p;
     p = take(cap * 64);                           if (c) c->cell_sums = (double*)p;
+    p = take(cap * 64);                           if (c) c->cell_sums2 = (double*)p;
+    p = take(cap * 32);                           if (c) c->cell_quad = (float4*)p;
     p = take((size_t)FF_DIRECT_SPLIT_ELEMS * 48); if (c) c->direct_part = (double*)p;
     for (int b = 0; b < 2; ++b) {
         p = take(n * 12);                         if (c) c->stage_pos2[b] = (float*)p;
@@ -141,7 +143,13 @@ extern "C" int ff_set_option(ff_ctx* c, int key, double value)
     case FF_OPT_TIMING: c->timing_enabled = value != 0.0; return FF_OK;
     case FF_OPT_GROUP:
         if (value != 32.0 && value != 64.0) return FF_ERR_INVALID_ARG;
+        if (value == 64.0 && c->order == 1) return FF_ERR_INVALID_ARG;      // the first-order walk exists for W = 32 only
         c->group = (int)value;
+        return FF_OK;
+    case FF_OPT_CELL_ORDER:
+        if (value != 0.0 && value != 1.0) return FF_ERR_INVALID_ARG;
+        if (value == 1.0 && c->group != 32) return FF_ERR_INVALID_ARG;
+        c->order = (int)value;
         return FF_OK;
     default: return FF_ERR_INVALID_ARG;
     }
@@ -333,6 +341,7 @@ extern "C" int ff_get_tree(ff_ctx* c, ff_tree_view* out)
     out->cell_first = c->cell_first; out->cell_end = c->cell_end; out->cell_level = c->cell_level;
     out->child = c->cell_child; out->leaf_count = c->leaf_count;
     out->cell_centre = (const float*)c->cell_centre; out->cell_moment = (const float*)c->cell_moment;
+    out->cell_quad = c->order == 1 ? (const float*)c->cell_quad : nullptr;
     return FF_OK;
 }
 

@@ -224,14 +224,28 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
 // fp64 sums in the fixed order of DESIGN.md (O4): children in octant order,
 // ((c0 + c1) + c2) + ...; a leaf's particles left to right; one fp64 divide and a
 // single rounding to fp32.
+// QUAD (FF_OPT_CELL_ORDER = 1): also the cell tensor D = sum_i (rho_i - rho') (x) u_i, symmetric part,
+// from six more fp64 sums of the symmetrised products rho_i (x) u_i in the same fixed order (O4b); every fp64
+// operation is an explicit round-to-nearest intrinsic so that no FMA contraction changes a bit against the oracle.
+__device__ __forceinline__ void ff_sym_products(const float4& p, const float4& m, double out[6])
+{
+    const double px = p.x, py = p.y, pz = p.z, ux = m.x, uy = m.y, uz = m.z;
+    out[0] = __dmul_rn(px, ux); out[1] = __dmul_rn(py, uy); out[2] = __dmul_rn(pz, uz);
+    out[3] = __dmul_rn(__dadd_rn(__dmul_rn(px, uy), __dmul_rn(py, ux)), 0.5);
+    out[4] = __dmul_rn(__dadd_rn(__dmul_rn(px, uz), __dmul_rn(pz, ux)), 0.5);
+    out[5] = __dmul_rn(__dadd_rn(__dmul_rn(py, uz), __dmul_rn(pz, uy)), 0.5);
+}
+
+template <bool QUAD>
 __global__ void __launch_bounds__(FF_MOM_THREADS)
 ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, int n, ff_globals* __restrict__ g,
              const int32_t* __restrict__ cell_first, const int32_t* __restrict__ cell_end,
              const int32_t* __restrict__ cell_list, const int32_t* __restrict__ cell_child,
              const int32_t* __restrict__ leaf_count, const float4* __restrict__ pos_s, float4* __restrict__ mom_s,
              double* __restrict__ sums, float4* __restrict__ centre,
-             float4* __restrict__ moment)
+             float4* __restrict__ moment, double* __restrict__ sums2, float4* __restrict__ quad)
 {
+    constexpr int NS = QUAD ? 12 : 6;                      // fp64 sums per cell
     cg::grid_group grid = cg::this_grid();
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
     for (int s = tid; s < n; s += nth) {
@@ -242,13 +256,13 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
     const int top = min(g->max_level, FF_MAX_LEVEL - 1);   // deepest level that holds an internal cell
     const float S = g->S;
     // Eight lanes per cell: lane o loads child o (one exposed memory latency per cell instead of eight),
-    // parks its six fp64 sums in shared memory, then lane a < 6 adds component a over the children in
+    // parks its fp64 sums in shared memory, then lane a < 6 adds component a (and a + 6) over the children in
     // octant order -- the same ((c0 + c1) + c2) + ... as a sequential loop.
-    __shared__ double sh[FF_MOM_THREADS / 8][8][6];
+    __shared__ double sh[FF_MOM_THREADS / 8][8][NS];
     const int o = threadIdx.x & 7;
     const unsigned gshift = (threadIdx.x & 24);            // first lane of this group inside the warp
     const unsigned gmask = 0xffu << gshift;
-    double(*mine)[6] = sh[threadIdx.x >> 3];
+    double(*mine)[NS] = sh[threadIdx.x >> 3];
     const int gid = tid >> 3, ngroups = nth >> 3;
     grid.sync();
     for (int level = top; level >= 0; --level) {
@@ -279,29 +293,49 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
                 for (int a = 0; a < 6; a += 2) {           // one 64-byte record per cell: u.xyz, p.xyz (two sectors)
                     const double2 v = *reinterpret_cast<const double2*>(sums + 8 * (size_t)e + a);
                     mine[o][a] = v.x; mine[o][a + 1] = v.y;
+                    if (QUAD) {
+                        const double2 q = *reinterpret_cast<const double2*>(sums2 + 8 * (size_t)e + a);
+                        mine[o][6 + a] = q.x; mine[o][7 + a] = q.y;
+                    }
                 }
             } else if (have) {
                 int slot = (int)((uint32_t)e & FF_CHILD_SLOT);
                 int cc = ((uint32_t)e & FF_CHILD_MULTI) ? leaf_count[slot] : 1;
                 float4 p = pos_s[slot], m = mom_s[slot];
-                double cu[3] = { m.x, m.y, m.z }, cp[3] = { p.x, p.y, p.z };
+                double cu[3] = { m.x, m.y, m.z }, cp[3] = { p.x, p.y, p.z }, cq[6];
+                if (QUAD) ff_sym_products(p, m, cq);
                 for (int j = slot + 1; j < slot + cc; ++j) {
                     p = pos_s[j]; m = mom_s[j];
                     cu[0] += (double)m.x; cu[1] += (double)m.y; cu[2] += (double)m.z;
                     cp[0] += (double)p.x; cp[1] += (double)p.y; cp[2] += (double)p.z;
+                    if (QUAD) {
+                        double pq[6];
+                        ff_sym_products(p, m, pq);
+#pragma unroll
+                        for (int a = 0; a < 6; ++a) cq[a] = __dadd_rn(cq[a], pq[a]);
+                    }
                 }
 #pragma unroll
                 for (int a = 0; a < 3; ++a) { mine[o][a] = cu[a]; mine[o][3 + a] = cp[a]; }
+                if (QUAD) {
+#pragma unroll
+                    for (int a = 0; a < 6; ++a) mine[o][6 + a] = cq[a];
+                }
             }
             const unsigned present = (__ballot_sync(gmask, have) >> gshift) & 0xffu;   // also orders the smem writes
             const double cnt = (double)(cell_end[id] - cell_first[id]);
-            double t = 0.0;
+            double t = 0.0, t2 = 0.0;
             if (o < 6) {
                 bool started = false;
 #pragma unroll
                 for (int c = 0; c < 8; ++c)
-                    if (present & (1u << c)) { t = started ? t + mine[c][o] : mine[c][o]; started = true; }
+                    if (present & (1u << c)) {
+                        t = started ? t + mine[c][o] : mine[c][o];
+                        if (QUAD) t2 = started ? __dadd_rn(t2, mine[c][6 + o]) : mine[c][6 + o];
+                        started = true;
+                    }
                 sums[8 * (size_t)id + o] = t;
+                if (QUAD) sums2[8 * (size_t)id + o] = t2;
             }
             float* cen = reinterpret_cast<float*>(centre + id);
             float* mo = reinterpret_cast<float*>(moment + id);
@@ -309,6 +343,17 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
             else if (o < 6) cen[o - 3] = (float)(t / cnt);
             else if (o == 6) cen[3] = s2;
             else mo[3] = (float)cnt;
+            if (QUAD) {
+                // lane c < 6 holds component c of D in the order xx yy zz xy xz yz = (ia, ib); su_a sits in lane a, sp_a
+                // in lane 3 + a of this group of eight
+                const int ia = o < 3 ? o : (o == 5 ? 1 : 0), ib = o < 3 ? o : (o == 3 ? 1 : 2);
+                const double su_a = __shfl_sync(gmask, t, ia, 8), su_b = __shfl_sync(gmask, t, ib, 8);
+                const double cen_a = __ddiv_rn(__shfl_sync(gmask, t, 3 + ia, 8), cnt);
+                const double cen_b = __ddiv_rn(__shfl_sync(gmask, t, 3 + ib, 8), cnt);
+                const double cu = o < 3 ? __dmul_rn(cen_a, su_b)
+                                        : __dmul_rn(__dadd_rn(__dmul_rn(cen_a, su_b), __dmul_rn(cen_b, su_a)), 0.5);
+                reinterpret_cast<float*>(quad + 2 * (size_t)id)[o] = o < 6 ? (float)__dsub_rn(t2, cu) : 0.0f;
+            }
             __syncwarp(gmask);                             // smem slots are reused by the group's next cell
         }
         if (level > FF_MOM_SOLO) grid.sync();
@@ -339,9 +384,12 @@ int ff_launch_build(ff_ctx* c)
 int ff_launch_moments(ff_ctx* c, const float* mom)
 {
     int n = (int)c->n;
-    int& per_sm = c->occ_moments;
+    const int quad = c->order == 1 ? 1 : 0;
+    const void* kernel = quad ? (const void*)ff_k_moments<true> : (const void*)ff_k_moments<false>;
+    int& per_sm = c->occ_moments[quad];
     if (!per_sm) {
-        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_moments, FF_MOM_THREADS, 0));
+        if (quad) FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_moments<true>, FF_MOM_THREADS, 0));
+        else FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_moments<false>, FF_MOM_THREADS, 0));
         if (per_sm < 1) return FF_ERR_CUDA;
     }
     int blocks = min((n + FF_MOM_THREADS - 1) / FF_MOM_THREADS, c->num_sms * min(per_sm, 8));
@@ -349,9 +397,8 @@ int ff_launch_moments(ff_ctx* c, const float* mom)
     void* args[] = { (void*)&mom, (void*)&perm, (void*)&n, (void*)&c->g, (void*)&c->cell_first, (void*)&c->cell_end,
                      (void*)&c->cell_list, (void*)&c->cell_child, (void*)&c->leaf_count, (void*)&c->pos_s,
                      (void*)&c->mom_s, (void*)&c->cell_sums, (void*)&c->cell_centre,
-                     (void*)&c->cell_moment };
-    FF_CUDA(c, cudaLaunchCooperativeKernel((const void*)ff_k_moments, dim3(blocks), dim3(FF_MOM_THREADS), args, 0,
-                                           c->stream));
+                     (void*)&c->cell_moment, (void*)&c->cell_sums2, (void*)&c->cell_quad };
+    FF_CUDA(c, cudaLaunchCooperativeKernel(kernel, dim3(blocks), dim3(FF_MOM_THREADS), args, 0, c->stream));
     c->launches++;
     return FF_OK;
 }

@@ -77,7 +77,8 @@ struct ff_ctx {
     int device;
     int num_sms;
     int group;                // targets per walk group W: 32 or 64 (FF_OPT_GROUP)
-    int occ_walk[8], occ_build, occ_moments;   // resident blocks per SM of the persistent / cooperative kernels (0 = not queried yet)
+    int order;                // 0 = the paper's cell (Eq. 14), 1 = plus the first-order cell term (FF_OPT_CELL_ORDER)
+    int occ_walk[12], occ_build, occ_moments[2];   // resident blocks per SM of the persistent / cooperative kernels (0 = not queried yet)
     cudaStream_t stream;
     // pipelined *_host calls: uploads on in_stream, compute on `stream`, downloads on out_stream, staging
     // buffers and events double-buffered by call parity (ff_api.cu)
@@ -102,6 +103,8 @@ struct ff_ctx {
     int32_t* cell_child;              // [cap][8]
     float4 *cell_centre, *cell_moment;
     double* cell_sums;                // [cap][8] fp64 sums in the fixed order: u.xyz, p.xyz, 2 pad (64-byte records)
+    double* cell_sums2;               // [cap][8] FF_OPT_CELL_ORDER = 1: sums of the symmetrised rho (x) u, xx yy zz xy xz yz, 2 pad
+    float4* cell_quad;                // [cap][2] the cell tensor D: (xx, yy, zz, xy) (xz, yz, 0, 0)
     double* direct_part;              // partial sums of the split direct kernel
     float *stage_pos2[2], *stage_mom2[2], *stage_H2[2], *stage_F2[2];   // device staging of the *_host calls
     float *stage_H, *stage_F;         // = stage_H2[0], stage_F2[0]: the fields of ff_step

@@ -94,6 +94,56 @@ __device__ __forceinline__ void ff_pair2_accum(const float4& A, const float2& B,
     s.sk = __fadd2_rn(s.sk, ca);
 }
 
+// ---- first-order cell term (FF_OPT_CELL_ORDER = 1) -------------------------
+// An accepted cell acts as its pseudo-particle (u', rho') PLUS the next term of the expansion of Eq. 11-12 about
+// rho', with the symmetric cell tensor D = sym sum_i (rho_i - rho') (x) u_i.  With R = rho_k - rho', t = tr D,
+// b = u_k.R, q = R.D.R, c1 = 3/R^5, c2 = 15/R^7, c3 = 105/R^9 the contracted first-order terms are
+//     dh = e R - 2 c1 D R,                                  e = c2 q - c1 t
+//     df = g R + 2 c2 b D R + e u_k - 2 (c1 D) u_k,         g = c2 (2 u_k.D.R + t b) - c3 b q
+// e u_k joins the scalar accumulator sk of the base term; sum_j c1 D_j is accumulated as a tensor and applied to u_k
+// once at the end.  49 more packed FP32 instructions per source and pair of targets.
+struct ff_accq2 {
+    float2 gxx, gyy, gzz, gxy, gxz, gyz;
+};
+__device__ __forceinline__ void ff_accq2_zero(ff_accq2& s) { s.gxx = s.gyy = s.gzz = s.gxy = s.gxz = s.gyz = ff_dup(0.0f); }
+
+// Q0 = Dxx, Dyy, Dzz, Dxy ; Q1 = Dxz, Dyz (a particle carries D = 0 and gets exactly nothing from this)
+__device__ __forceinline__ void ff_pair2_quad(const float4& A, const float2& B, const float4& Q0, const float2& Q1,
+                                              const ff_target2& t, ff_acc2& s, ff_accq2& sq)
+{
+    float2 dx, dy, dz, r2;
+    ff_pair2_geom(A, t, dx, dy, dz, r2);
+    const float2 rinv = ff_rsqrt2(r2);
+    ff_pair2_accum(A, B, t, dx, dy, dz, rinv, s);
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 nr3 = __fmul2_rn(rinv2, make_float2(-rinv.x, -rinv.y));
+    const float2 c1 = __fmul2_rn(nr3, __fmul2_rn(rinv2, ff_dup(-3.0f)));           // 3 / R^5
+    const float2 c2 = __fmul2_rn(__fmul2_rn(c1, rinv2), ff_dup(5.0f));             // 15 / R^7
+    const float2 c3 = __fmul2_rn(__fmul2_rn(c2, rinv2), ff_dup(7.0f));             // 105 / R^9
+    const float2 b = __ffma2_rn(t.uz, dz, __ffma2_rn(t.uy, dy, __fmul2_rn(t.ux, dx)));
+    const float2 Dxx = ff_dup(Q0.x), Dyy = ff_dup(Q0.y), Dzz = ff_dup(Q0.z), Dxy = ff_dup(Q0.w), Dxz = ff_dup(Q1.x),
+                 Dyz = ff_dup(Q1.y);
+    const float2 vx = __ffma2_rn(Dxz, dz, __ffma2_rn(Dxy, dy, __fmul2_rn(Dxx, dx)));   // D R
+    const float2 vy = __ffma2_rn(Dyz, dz, __ffma2_rn(Dyy, dy, __fmul2_rn(Dxy, dx)));
+    const float2 vz = __ffma2_rn(Dzz, dz, __ffma2_rn(Dyz, dy, __fmul2_rn(Dxz, dx)));
+    const float2 q = __ffma2_rn(vz, dz, __ffma2_rn(vy, dy, __fmul2_rn(vx, dx)));       // R.D.R
+    const float2 uv = __ffma2_rn(vz, t.uz, __ffma2_rn(vy, t.uy, __fmul2_rn(vx, t.ux)));   // u_k.D.R
+    const float2 tr = __fadd2_rn(__fadd2_rn(Dxx, Dyy), Dzz);
+    const float2 c1t = __fmul2_rn(c1, tr);
+    const float2 e = __ffma2_rn(c2, q, make_float2(-c1t.x, -c1t.y));
+    const float2 m2c1 = __fmul2_rn(c1, ff_dup(-2.0f));
+    s.hx = __ffma2_rn(e, dx, s.hx); s.hy = __ffma2_rn(e, dy, s.hy); s.hz = __ffma2_rn(e, dz, s.hz);
+    s.hx = __ffma2_rn(m2c1, vx, s.hx); s.hy = __ffma2_rn(m2c1, vy, s.hy); s.hz = __ffma2_rn(m2c1, vz, s.hz);
+    const float2 c3bq = __fmul2_rn(c3, __fmul2_rn(b, q));
+    const float2 gg = __ffma2_rn(c2, __ffma2_rn(ff_dup(2.0f), uv, __fmul2_rn(tr, b)), make_float2(-c3bq.x, -c3bq.y));
+    const float2 c2b2 = __fmul2_rn(__fmul2_rn(c2, b), ff_dup(2.0f));
+    s.fx = __ffma2_rn(gg, dx, s.fx); s.fy = __ffma2_rn(gg, dy, s.fy); s.fz = __ffma2_rn(gg, dz, s.fz);
+    s.fx = __ffma2_rn(c2b2, vx, s.fx); s.fy = __ffma2_rn(c2b2, vy, s.fy); s.fz = __ffma2_rn(c2b2, vz, s.fz);
+    s.sk = __fadd2_rn(s.sk, e);
+    sq.gxx = __ffma2_rn(c1, Dxx, sq.gxx); sq.gyy = __ffma2_rn(c1, Dyy, sq.gyy); sq.gzz = __ffma2_rn(c1, Dzz, sq.gzz);
+    sq.gxy = __ffma2_rn(c1, Dxy, sq.gxy); sq.gxz = __ffma2_rn(c1, Dxz, sq.gxz); sq.gyz = __ffma2_rn(c1, Dyz, sq.gyz);
+}
+
 // one source against the lane's two targets, nothing masked (the hot loop of the walk and of the direct kernel)
 __device__ __forceinline__ void ff_pair2(const float4& A, const float2& B, const ff_target2& t, ff_acc2& s)
 {

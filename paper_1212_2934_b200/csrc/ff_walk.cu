@@ -31,11 +31,13 @@
 #include "ff_internal.cuh"
 #include "ff_pair.cuh"
 
-template <int W>
+template <int W, bool QUAD>
 struct ff_walk_smem {
     int32_t stack[FF_WALK_STACK];
     float4 pendA[FF_WALK_PEND];        // ring entry e: x, y, z, mx
     float2 pendB[FF_WALK_PEND];        //               my, mz
+    float4 pendQ0[QUAD ? FF_WALK_PEND : 1];   // FF_OPT_CELL_ORDER = 1: the cell tensor Dxx, Dyy, Dzz, Dxy
+    float2 pendQ1[QUAD ? FF_WALK_PEND : 1];   //                                         Dxz, Dyz  (0 for a particle)
     float4 mem_xy[W / 2];              // group members in pairs (pair m = members 2m, 2m + 1): x0,x1,y0,y1
     float2 mem_z[W / 2];               //                                                        z0,z1
     float4 mem_uxy[W / 2];             // their moments, same layout: ux0,ux1,uy0,uy1
@@ -47,15 +49,15 @@ struct ff_walk_smem {
 };
 
 // one group of W consecutive sorted targets, walked by one warp
-template <int W, bool COUNT, bool BUCKET>
+template <int W, bool COUNT, bool BUCKET, bool QUAD>
 __device__ __forceinline__ void
-ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
+ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
           int n, float theta, const int n_cells, const float4* __restrict__ pos_s,
           const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
           const int4* __restrict__ cell_info, const int4* __restrict__ cell_child,
           const int32_t* __restrict__ leaf_count, const float4* __restrict__ centre,
-          const float4* __restrict__ moment, float* __restrict__ H_out, float* __restrict__ F_out,
-          unsigned long long* __restrict__ counters)
+          const float4* __restrict__ moment, const float4* __restrict__ quad, float* __restrict__ H_out,
+          float* __restrict__ F_out, unsigned long long* __restrict__ counters)
 {
     constexpr int ST = (W == 32) ? 2 : 1;                  // ring entries per evaluation step of one lane
     constexpr int BATCH_ITERS = 32 / ST;                   // evaluation steps per batch of 32 ring entries
@@ -82,6 +84,7 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
             sm.pendA[i] = make_float4(p.x, p.y, p.z, u.x);
             sm.pendB[i] = make_float2(u.y, u.z);
         };
+        (void)quad;
         const int ma = g0 + min(lane, nm - 1), mb = g0 + min(lane + 32, nm - 1);
         const float4 pa = __ldg(pos_s + ma), ua = __ldg(mom_s + ma);
         const float4 pb = (W == 64) ? __ldg(pos_s + mb) : pa, ub = (W == 64) ? __ldg(mom_s + mb) : ua;
@@ -127,6 +130,8 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
     }
     ff_acc2 s;
     ff_acc2_zero(s);
+    ff_accq2 sq;
+    ff_accq2_zero(sq);
     __syncwarp();
     // the group's own members: direct terms, self skipped by index (Alg. 1 line 5);
     // slots >= nm of a ragged last group hold copies of the last member and are masked the same way
@@ -154,7 +159,16 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
         __syncwarp();
         const float4* qa = sm.pendA + pend_head + half;
         const float2* qb = sm.pendB + pend_head + half;
-        if (iters == BATCH_ITERS) {
+        if (QUAD) {
+            const float4* q0 = sm.pendQ0 + pend_head + half;
+            const float2* q1 = sm.pendQ1 + pend_head + half;
+            if (iters == BATCH_ITERS) {
+#pragma unroll 2
+                for (int i = 0; i < BATCH_ITERS; ++i) ff_pair2_quad(qa[ST * i], qb[ST * i], q0[ST * i], q1[ST * i], tg, s, sq);
+            } else {
+                for (int i = 0; i < iters; ++i) ff_pair2_quad(qa[ST * i], qb[ST * i], q0[ST * i], q1[ST * i], tg, s, sq);
+            }
+        } else if (iters == BATCH_ITERS) {
 #pragma unroll 4
             for (int i = 0; i < BATCH_ITERS; ++i) ff_pair2(qa[ST * i], qb[ST * i], tg, s);
         } else {
@@ -163,12 +177,13 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
         __syncwarp();
     };
     // append the lanes with `take` set (A = x, y, z, mx; B = my, mz) to the ring
-    auto append = [&](bool take, const float4& A, const float2& B) {
+    auto append = [&](bool take, const float4& A, const float2& B, const float4& Q0, const float2& Q1) {
         const unsigned m = __ballot_sync(FF_FULL, take);
         if (take) {
             const int slot = (pend_head + pend_cnt + __popc(m & lt)) & (FF_WALK_PEND - 1);
             sm.pendA[slot] = A;
             sm.pendB[slot] = B;
+            if (QUAD) { sm.pendQ0[slot] = Q0; sm.pendQ1[slot] = Q1; }
         }
         pend_cnt += __popc(m);
     };
@@ -186,7 +201,8 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
             const bool ok = j < first + cnt && !(j >= g0 && j < g1);
             float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = A;
             if (ok) { A = __ldg(pos_s + j); B = __ldg(mom_s + j); }
-            append(ok, make_float4(A.x, A.y, A.z, B.x), make_float2(B.y, B.z));
+            append(ok, make_float4(A.x, A.y, A.z, B.x), make_float2(B.y, B.z), make_float4(0.f, 0.f, 0.f, 0.f),
+                   make_float2(0.f, 0.f));
             if (COUNT) c_part += (unsigned long long)__popc(__ballot_sync(FF_FULL, ok)) * nm;
             drain();
         }
@@ -293,7 +309,16 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
             if (park) sm.amb[amb_cnt + __popc(pm & lt)] = e;
             amb_cnt += __popc(pm);
         }
-        append(take, make_float4(A.x, A.y, A.z, B.x), make_float2(B.y, B.z));
+        {
+            float4 Q0 = make_float4(0.f, 0.f, 0.f, 0.f);
+            float2 Q1 = make_float2(0.f, 0.f);
+            if (QUAD && accept_cell) {
+                Q0 = __ldg(quad + 2 * (size_t)e);
+                const float4 t4 = __ldg(quad + 2 * (size_t)e + 1);
+                Q1 = make_float2(t4.x, t4.y);
+            }
+            append(take, make_float4(A.x, A.y, A.z, B.x), make_float2(B.y, B.z), Q0, Q1);
+        }
         // the children of an opened cell: the non-empty sub-cells, compacted to the front of its eight links
         int4 c0 = make_int4(-1, -1, -1, -1), c1 = c0;
         int nch = 0;
@@ -351,6 +376,10 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
                 const float4 last = sm.pendA[pend_head + pend_cnt - 1];
                 sm.pendA[pend_head + pend_cnt] = make_float4(last.x, last.y, last.z, 0.f);
                 sm.pendB[pend_head + pend_cnt] = make_float2(0.f, 0.f);
+                if (QUAD) {
+                    sm.pendQ0[pend_head + pend_cnt] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    sm.pendQ1[pend_head + pend_cnt] = make_float2(0.f, 0.f);
+                }
             }
         }
         eval((pend_cnt + ST - 1) / ST);
@@ -360,7 +389,16 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
     if (W == 32) {
 #define FF_FOLD(v) v.x += __shfl_xor_sync(FF_FULL, v.x, 16); v.y += __shfl_xor_sync(FF_FULL, v.y, 16)
         FF_FOLD(s.hx); FF_FOLD(s.hy); FF_FOLD(s.hz); FF_FOLD(s.fx); FF_FOLD(s.fy); FF_FOLD(s.fz); FF_FOLD(s.sk);
+        if (QUAD) { FF_FOLD(sq.gxx); FF_FOLD(sq.gyy); FF_FOLD(sq.gzz); FF_FOLD(sq.gxy); FF_FOLD(sq.gxz); FF_FOLD(sq.gyz); }
 #undef FF_FOLD
+    }
+    if (QUAD) {
+        // df also holds -2 (sum_j c1 D_j) u_k: the accumulated tensor applied to the target's moment once
+        const float2 m2 = ff_dup(-2.0f);
+        const float2 gx = __ffma2_rn(sq.gxz, tg.uz, __ffma2_rn(sq.gxy, tg.uy, __fmul2_rn(sq.gxx, tg.ux)));
+        const float2 gy = __ffma2_rn(sq.gyz, tg.uz, __ffma2_rn(sq.gyy, tg.uy, __fmul2_rn(sq.gxy, tg.ux)));
+        const float2 gz = __ffma2_rn(sq.gzz, tg.uz, __ffma2_rn(sq.gyz, tg.uy, __fmul2_rn(sq.gxz, tg.ux)));
+        s.fx = __ffma2_rn(m2, gx, s.fx); s.fy = __ffma2_rn(m2, gy, s.fy); s.fz = __ffma2_rn(m2, gz, s.fz);
     }
     // (the moments are read back from the packed target registers: keeping the loaded float4 alive across the
     // walk makes ptxas rebuild the register pairs with MOVs inside the evaluation loop)
@@ -392,18 +430,18 @@ ff_walk_group(ff_walk_smem<W>& sm, const int grp, const int lane,
 // Persistent launch: every warp fetches the next group from a device-wide counter (g->walk_next,
 // zeroed by the last cell-moment launch), so no SM idles while one block's slowest group finishes
 // and consecutive (spatially adjacent) groups run at the same time and share cells in L1/L2.
-template <int W, bool COUNT, bool BUCKET>
-__global__ void __launch_bounds__(FF_WALK_WARPS * 32, FF_WALK_MINB)
+template <int W, bool COUNT, bool BUCKET, bool QUAD>
+__global__ void __launch_bounds__(FF_WALK_WARPS * 32, QUAD ? 4 : FF_WALK_MINB)
 ff_k_walk(int n, int group_begin, int group_end, float theta, ff_globals* __restrict__ g, const float4* __restrict__ pos_s,
           const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
           const int4* __restrict__ cell_info, const int4* __restrict__ cell_child,
           const int32_t* __restrict__ leaf_count, const float4* __restrict__ centre,
-          const float4* __restrict__ moment, float* __restrict__ H_out, float* __restrict__ F_out,
-          unsigned long long* __restrict__ counters)
+          const float4* __restrict__ moment, const float4* __restrict__ quad, float* __restrict__ H_out,
+          float* __restrict__ F_out, unsigned long long* __restrict__ counters)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    ff_walk_smem<W>& sm = reinterpret_cast<ff_walk_smem<W>*>(smem_raw)[w];
+    ff_walk_smem<W, QUAD>& sm = reinterpret_cast<ff_walk_smem<W, QUAD>*>(smem_raw)[w];
     const int groups = group_end;                          // groups [group_begin, group_end) of the sorted order
     const int n_cells = g->n_cells;
     for (;;) {
@@ -411,30 +449,30 @@ ff_k_walk(int n, int group_begin, int group_end, float theta, ff_globals* __rest
         if (lane == 0) grp = group_begin + atomicAdd(&g->walk_next, 1);
         grp = __shfl_sync(FF_FULL, grp, 0);
         if (grp >= groups) break;
-        ff_walk_group<W, COUNT, BUCKET>(sm, grp, lane, n, theta, n_cells, pos_s, mom_s, perm, cell_info, cell_child,
-                                        leaf_count, centre, moment, H_out, F_out, counters);
+        ff_walk_group<W, COUNT, BUCKET, QUAD>(sm, grp, lane, n, theta, n_cells, pos_s, mom_s, perm, cell_info, cell_child,
+                                              leaf_count, centre, moment, quad, H_out, F_out, counters);
         __syncwarp();
     }
 }
 
-template <int W, bool COUNT, bool BUCKET>
+template <int W, bool COUNT, bool BUCKET, bool QUAD>
 static int ff_launch_walk_t(ff_ctx* c, float* H_out, float* F_out, int group_begin, int group_end, int variant)
 {
     const int n = (int)c->n;
     const int groups = group_end - group_begin;
-    const size_t smem = sizeof(ff_walk_smem<W>) * FF_WALK_WARPS;
+    const size_t smem = sizeof(ff_walk_smem<W, QUAD>) * FF_WALK_WARPS;
     int& per_sm = c->occ_walk[variant];                    // per context: contexts may live on different devices
     if (!per_sm) {
-        FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<W, COUNT, BUCKET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_walk<W, COUNT, BUCKET>, FF_WALK_WARPS * 32, smem));
+        FF_CUDA(c, cudaFuncSetAttribute(ff_k_walk<W, COUNT, BUCKET, QUAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_walk<W, COUNT, BUCKET, QUAD>, FF_WALK_WARPS * 32, smem));
         if (per_sm < 1) return FF_ERR_CUDA;
     }
     const int blocks = min(c->num_sms * per_sm, (groups + FF_WALK_WARPS - 1) / FF_WALK_WARPS);
     if (COUNT) FF_CUDA(c, cudaMemsetAsync(c->g->counters, 0, sizeof(c->g->counters), c->stream));
-    auto kernel = ff_k_walk<W, COUNT, BUCKET>;
+    auto kernel = ff_k_walk<W, COUNT, BUCKET, QUAD>;
     FF_LAUNCH(c, kernel, blocks, FF_WALK_WARPS * 32, smem, n, group_begin, group_end, c->theta, c->g,
               c->pos_s, c->mom_s, c->idx[0], c->cell_info, (const int4*)c->cell_child, c->leaf_count, c->cell_centre,
-              c->cell_moment, H_out, F_out, c->g->counters);
+              c->cell_moment, c->cell_quad, H_out, F_out, c->g->counters);
     return FF_OK;
 }
 
@@ -444,15 +482,19 @@ int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out, int group_begin, int g
     if (group_end < 0) group_end = (n + W - 1) / W;
     if (group_end - group_begin <= 0) return FF_OK;
     const int cnt = c->count_enabled ? 1 : 0, bucket = c->nleaf > 1 ? 1 : 0;
-    const int variant = (W == 64 ? 4 : 0) + 2 * cnt + bucket;
+    const int variant = (W == 64 ? 4 : (c->order == 1 ? 8 : 0)) + 2 * cnt + bucket;
     switch (variant) {
-    case 0: return ff_launch_walk_t<32, false, false>(c, H_out, F_out, group_begin, group_end, variant);
-    case 1: return ff_launch_walk_t<32, false, true>(c, H_out, F_out, group_begin, group_end, variant);
-    case 2: return ff_launch_walk_t<32, true, false>(c, H_out, F_out, group_begin, group_end, variant);
-    case 3: return ff_launch_walk_t<32, true, true>(c, H_out, F_out, group_begin, group_end, variant);
-    case 4: return ff_launch_walk_t<64, false, false>(c, H_out, F_out, group_begin, group_end, variant);
-    case 5: return ff_launch_walk_t<64, false, true>(c, H_out, F_out, group_begin, group_end, variant);
-    case 6: return ff_launch_walk_t<64, true, false>(c, H_out, F_out, group_begin, group_end, variant);
-    default: return ff_launch_walk_t<64, true, true>(c, H_out, F_out, group_begin, group_end, variant);
+    case 0: return ff_launch_walk_t<32, false, false, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 1: return ff_launch_walk_t<32, false, true, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 2: return ff_launch_walk_t<32, true, false, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 3: return ff_launch_walk_t<32, true, true, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 4: return ff_launch_walk_t<64, false, false, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 5: return ff_launch_walk_t<64, false, true, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 6: return ff_launch_walk_t<64, true, false, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 7: return ff_launch_walk_t<64, true, true, false>(c, H_out, F_out, group_begin, group_end, variant);
+    case 8: return ff_launch_walk_t<32, false, false, true>(c, H_out, F_out, group_begin, group_end, variant);
+    case 9: return ff_launch_walk_t<32, false, true, true>(c, H_out, F_out, group_begin, group_end, variant);
+    case 10: return ff_launch_walk_t<32, true, false, true>(c, H_out, F_out, group_begin, group_end, variant);
+    default: return ff_launch_walk_t<32, true, true, true>(c, H_out, F_out, group_begin, group_end, variant);
     }
 }

@@ -193,6 +193,45 @@ def test_group_width_64(ff, N, nleaf, theta, cfg):
     assert ctx.counters() == cnt32
 
 
+@pytest.mark.parametrize("N,nleaf,theta,cfg", [(4096, 1, 0.5, 1), (2, 1, 0.5, 1), (33, 1, 0.7, 1), (1000, 1, 0.3, 1),
+                                                (4097, 4, 0.6, 1), (3000, 1, 0.5, 4), (2500, 16, 1.0, 2), (6000, 1, 0.8, 2)])
+def test_first_order_cell_term(ff, N, nleaf, theta, cfg):
+    """FF_OPT_CELL_ORDER = 1: every accepted cell contributes its pseudo-particle plus the first-order
+    term with the cell tensor D.  Same interaction lists as order 0 (counters equal the oracle's), D bit-exact against
+    the oracle's node data, H and F within 1e-4 of the oracle's order-1 evaluation."""
+    c = ffgen.config(cfg, N=N, seed=N)
+    pos, mom = c["pos"], c["mom"]
+    ctx = ff.FFContext(N, theta, nleaf=nleaf, counters=True)
+    ctx.set_option(ff.FF_OPT_CELL_ORDER, 1)
+    p, m = _dev(pos), _dev(mom)
+    ctx.build_tree(p)
+    H, F = ctx.eval_bh(p, m)
+    H, F = H.cpu().numpy(), F.cpu().numpy()
+    Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, theta, 32, nleaf=nleaf, scale=True, order=1)
+    om = otree.moments(mom)
+    _check_tree(ff, ctx, otree, om)
+    assert ctx.counters() == cnt
+    t = ctx.get_tree()
+    nd = otree.nodes()
+    idx = {(int(f), int(l)): i for i, (f, l, leaf) in enumerate(zip(nd["first"], nd["level"], nd["is_leaf"])) if not leaf}
+    sel = np.array([idx[(int(f), int(l))] for f, l in zip(t["cell_first"], t["cell_level"])], dtype=np.int64)
+    if len(sel):
+        assert np.array_equal(t["cell_quad"][:, :6], om["dsym"][sel]) and np.all(t["cell_quad"][:, 6:] == 0)
+    check_hf(H, F, Ho, Fo, Q, TOL_BH, survey=cfg != 4)
+    # the correction is not a no-op, and switching it off again restores the paper's cell
+    H0o, _, _, _ = oracle.barnes_hut(pos, mom, theta, 32, nleaf=nleaf)
+    if cnt[0] > 0:
+        assert not np.allclose(Ho, H0o, rtol=1e-6, atol=0)
+    ctx.set_option(ff.FF_OPT_CELL_ORDER, 0)
+    H0, _ = ctx.eval_bh(p, m)
+    assert rel_err(H0.cpu().numpy(), H0o)[3] < 1e-5 and "cell_quad" not in ctx.get_tree()
+    with pytest.raises(ff.FFError):
+        ctx.set_option(ff.FF_OPT_CELL_ORDER, 2)
+    ctx.set_option(ff.FF_OPT_GROUP, 64)
+    with pytest.raises(ff.FFError):
+        ctx.set_option(ff.FF_OPT_CELL_ORDER, 1)                  # the first-order walk exists for W = 32 only
+
+
 def test_skipping_one_output_leaves_the_other_unchanged(ff, cfg1):
     """H_out / F_out = NULL (include/ff.h: "either may be NULL to skip it") on both evaluators: the output that is
     asked for equals, bit for bit, the one of the call that asks for both, and nothing else is written."""
