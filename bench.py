@@ -541,6 +541,7 @@ def run_ours(args):
                                     "extrapolated_s_per_eval": t_ap * N / len(tsel),
                                     "sample": "%d targets x all sources, fp64" % len(tsel)}})
         errs = {}
+        ctx.build_tree(pos)          # (the host calls above built their tree from the staging copy of the positions)
         for th in (0.3, 0.5, 0.7):
             ctx.set_option(ff.FF_OPT_THETA, th)
             Hb, Fb = ctx.eval_bh(pos, mom)
@@ -571,6 +572,39 @@ def run_ours(args):
             "H_rel_l2_vs_allpairs": float((Hb - Hd).double().norm() / Hd.double().norm()),
             "F_rel_l2_vs_allpairs": float((Fb - Fd).double().norm() / Fd.double().norm()),
             "note": "FF_OPT_GROUP = 64 at theta = %g, L2 not flushed; W = 32 is the headline" % theta}
+
+        # better cells at equal cost: bucket leaves and the first-order cell term, alone and together
+        variants = {}
+        for nleaf_v, order_v, th in ((1, 0, 0.5), (1, 1, 0.5), (8, 0, 0.5), (8, 1, 0.5), (1, 1, 0.6), (8, 1, 0.6),
+                                     (1, 0, 0.7), (1, 1, 0.7), (8, 1, 0.7), (1, 0, 0.4)):
+            ctx.set_option(ff.FF_OPT_NLEAF, nleaf_v)
+            ctx.set_option(ff.FF_OPT_CELL_ORDER, order_v)
+            ctx.set_option(ff.FF_OPT_THETA, th)
+            ctx.set_option(ff.FF_OPT_COUNTERS, 1)
+            ctx.build_tree(pos)
+            Hb, Fb = ctx.eval_bh(pos, mom)
+            cv = ctx.counters()
+            ctx.set_option(ff.FF_OPT_COUNTERS, 0)
+            ctx.timings()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(5):
+                ctx.build_tree(pos)
+                ctx.eval_bh(pos, mom, Hb, Fb)
+            b.record()
+            b.synchronize()
+            variants["nleaf=%d order=%d theta=%g" % (nleaf_v, order_v, th)] = {
+                "ms_per_step": a.elapsed_time(b) / 5, "walk_ms": ctx.timings()["walk"],
+                "cell_terms_per_target": cv[0] / N, "particle_terms_per_target": cv[1] / N,
+                "H_rel_l2_vs_allpairs": float((Hb - Hd).double().norm() / Hd.double().norm()),
+                "F_rel_l2_vs_allpairs": float((Fb - Fd).double().norm() / Fd.double().norm())}
+        ctx.set_option(ff.FF_OPT_NLEAF, 1)
+        ctx.set_option(ff.FF_OPT_CELL_ORDER, 0)
+        ctx.set_option(ff.FF_OPT_THETA, theta)
+        extras["cell_variants"] = {"by_variant": variants,
+                                   "note": "config 3, L2 not flushed; order=1 adds the first-order cell term "
+                                           "(FF_OPT_CELL_ORDER), nleaf=8 bucket leaves (FF_OPT_NLEAF); errors are global "
+                                           "relative L2 against the GPU all-pairs result"}
 
         # the same recipe at smaller sizes (device-resident, L2 not flushed): how the step scales with N
         sweep = {}

@@ -3,7 +3,8 @@
     compute-sanitizer --tool memcheck  python tests/sanitizer_smoke.py
     compute-sanitizer --tool racecheck python tests/sanitizer_smoke.py
 
-Covers ff_build_tree, ff_eval_bh (N_leaf 1 and 4, ragged N, counters on and off, W = 32 and 64), ff_eval_bh_range,
+Covers ff_build_tree, ff_eval_bh (N_leaf 1, 2 and 4, ragged N, counters on and off, W = 32 and 64, cell order 0 and 1),
+ff_eval_bh_range,
 ff_eval_direct (split and unsplit grids), ff_eval_bh_host and ff_step with Lennard-Jones pairs + walls, Barnes-Hut
 and all-pairs.  The hazards it is there for: the walk's shared-memory ring, stack and parked-cell queue are ordered
 by __syncwarp only, the sort's look-back by volatile status words (the paper's own build relies on atomics used as
@@ -22,12 +23,14 @@ import paper_1212_2934_b200 as ff
 
 
 def main():
-    for N, nleaf, group in ((3000, 1, 32), (4097, 4, 32), (33, 1, 32), (2500, 1, 64)):
+    for N, nleaf, group, order in ((3000, 1, 32, 0), (4097, 4, 32, 0), (33, 1, 32, 0), (2500, 1, 64, 0), (2100, 2, 32, 1)):
         c = ffgen.config(1, N=N)
         pos, mom = torch.from_numpy(c["pos"]).cuda(), torch.from_numpy(c["mom"]).cuda()
         ctx = ff.FFContext(N, 0.5, nleaf=nleaf, counters=True)
         if group != 32:
             ctx.set_option(ff.FF_OPT_GROUP, group)
+        if order:
+            ctx.set_option(ff.FF_OPT_CELL_ORDER, order)
         ctx.build_tree(pos)
         H, F = ctx.eval_bh(pos, mom)
         ctx.set_option(ff.FF_OPT_COUNTERS, 0)
@@ -54,8 +57,8 @@ def main():
                 ctx.step(x, v, u, w, p, s)
         torch.cuda.synchronize()
         same = bool(torch.equal(H, H2) and torch.equal(F, F2))
-        print("N=%d nleaf=%d W=%d: ranges compose=%s, BH vs direct rel L2 %.3e, finite=%s"
-              % (N, nleaf, group, same, float((H - Hd).norm() / Hd.norm()), bool(torch.isfinite(x).all())))
+        print("N=%d nleaf=%d W=%d order=%d: ranges compose=%s, BH vs direct rel L2 %.3e, finite=%s"
+              % (N, nleaf, group, order, same, float((H - Hd).norm() / Hd.norm()), bool(torch.isfinite(x).all())))
         assert same
 
 
