@@ -29,7 +29,7 @@ static size_t carve(ff_ctx* c, char* base, int64_t N)
     p = take(n * 16);                             if (c) c->mom_s = (float4*)p;
     p = take(n * 4);                              if (c) c->leaf_count = (int32_t*)p;
     p = take(n * 4);                              if (c) c->cell_base = (int32_t*)p;
-    p = take((scan_tiles + 1) * 4);               if (c) c->scan_blk = (uint32_t*)p;
+    p = take((scan_tiles + 1 + FF_BUILD_MAX_BLOCKS) * 4); if (c) c->scan_blk = (uint32_t*)p;   // one word per block of ff_k_build
     p = take(sort_tiles * FF_RADIX * 4 * FF_SORT_PASSES); if (c) c->sort_status = (uint32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_first = (int32_t*)p;
     p = take(cap * 4);                            if (c) c->cell_end = (int32_t*)p;
@@ -172,6 +172,7 @@ extern "C" int ff_build_tree(ff_ctx* c, const float* pos, int64_t n)
     ff_phase_begin(c, FF_PH_BUILD);
     if ((rc = ff_launch_build(c)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_BUILD);
+    c->globals_clean = 1;                                  // ff_k_build leaves the reset state for the next build
     c->tree_built = 1;
     c->tree_pos = pos;
     return FF_OK;

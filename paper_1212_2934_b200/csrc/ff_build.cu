@@ -57,14 +57,22 @@ __device__ __forceinline__ int ff_gallop_bound(const uint32_t* __restrict__ key,
 //   phase 1  every block counts the cells that start in its contiguous range of slots
 //   phase 2  exclusive scan (block prefix + in-tile scan) -> cell_base[slot]; every cell gets
 //            its first slot and level; level histogram
-//   phase 3  eight lanes per cell: lane o finds the end of octant o with a galloping search in
-//            the sorted keys (one search per lane, all of similar length), which gives the cell's
-//            range and its child links (non-empty sub-cells compacted to the front, in octant
-//            order); the cell's id is appended to its level's list
-//            (ff_k_moments walks the levels deepest first)
+//   phase 3  eight lanes per cell (lane o = octant o).  The group reads a WINDOW of the 32 sorted
+//            keys that follow the cell's first slot in one coalesced step and counts, per octant
+//            bound, the window keys below it (byte counters packed in two words, summed over the
+//            eight lanes with three shuffles): for the ~95 % of the cells that hold <= 32
+//            particles this gives every child boundary after ONE memory latency.  An octant whose
+//            end lies beyond the window falls back to a galloping search from the window's end.
+//            Then range and child links (non-empty sub-cells compacted to the front, in octant
+//            order); the cell's id is appended to its level's list (ff_k_moments walks the levels
+//            deepest first).
 // The paper builds the tree by locked insertion (kernel 2); no locks here, and
 // the result does not depend on scheduling except for the order inside a level list, which no
 // result depends on.
+#define FF_BUILD_WINDOW 32
+#ifndef FF_BUILD_CELLS
+#define FF_BUILD_CELLS 4                  // cells a group of eight lanes has in flight (phase 3)
+#endif
 __global__ void __launch_bounds__(FF_BUILD_THREADS)
 ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restrict__ blk,
            int32_t* __restrict__ cell_base, int32_t* __restrict__ cell_first, int32_t* __restrict__ cell_end,
@@ -79,6 +87,10 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
     const int tiles = (n + FF_BUILD_TILE - 1) / FF_BUILD_TILE;
     const int tpb = (tiles + gridDim.x - 1) / gridDim.x;
     const int t0 = min(tiles, (int)blockIdx.x * tpb), t1 = min(tiles, t0 + tpb);
+#ifdef FF_BUILD_PROFILE
+    unsigned long long tq[4];
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tq[0]));
+#endif
 
     // ---- phase 1
     {
@@ -99,7 +111,13 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
             blk[blockIdx.x] = t;
         }
     }
+    // the state the NEXT ff_build_tree starts from (bounding box, sort tickets and digit histograms are all consumed
+    // by now): saves a reset launch per step; ff_create and a failed call run ff_k_reset instead
+    if (blockIdx.x == gridDim.x - 1) ff_reset_globals(g, threadIdx.x, FF_BUILD_THREADS);
     grid.sync();
+#ifdef FF_BUILD_PROFILE
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tq[1]));
+#endif
 
     // ---- phase 2
     {
@@ -149,7 +167,7 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
                 if (i < n) cell_base[i] = (int32_t)run;
                 if (fits)
                     for (uint32_t q = 0; q < c[r]; ++q) {
-                        int l = lp[r] + 1 + (int)q;
+                        const int l = lp[r] + 1 + (int)q;
                         cell_first[run + q] = i;
                         cell_level[run + q] = l;
                         atomicAdd(&s_hist[l], 1);
@@ -162,9 +180,21 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
         if (threadIdx.x < FF_MAX_LEVEL && s_hist[threadIdx.x]) atomicAdd(&g->level_count[threadIdx.x], s_hist[threadIdx.x]);
     }
     grid.sync();
+#ifdef FF_BUILD_PROFILE
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tq[2]));
+#endif
 
     // ---- phase 3
+    // Latency bound (three dependent loads per cell: first slot -> window keys -> cell_base of the children), so every
+    // group of eight lanes works on FF_BUILD_CELLS cells at a time and issues each stage's loads for all of them together.
     const int n_cells = g->n_cells;
+    const int o = threadIdx.x & 7;
+    const int gsh = threadIdx.x & 24;
+    const unsigned gmask = 0xffu << gsh;
+    const int stride = gridDim.x * (FF_BUILD_THREADS / 8);
+    const int id0 = blockIdx.x * (FF_BUILD_THREADS / 8) + (threadIdx.x >> 3);
+    // cell ids grouped by level (ff_k_moments walks the levels deepest first): start of every level's list, then
+    // the block reserves, per level, room for the cells it is about to handle (one global atomic per level and block)
     __syncthreads();
     if (threadIdx.x == 0) {
         int run = 0, deepest = 0;
@@ -179,42 +209,95 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
     }
     if (threadIdx.x < FF_MAX_LEVEL) s_hist[threadIdx.x] = 0;
     __syncthreads();
-    const int cpb = (n_cells + gridDim.x - 1) / gridDim.x;
-    const int c0 = min(n_cells, (int)blockIdx.x * cpb), c1 = min(n_cells, c0 + cpb);
-    for (int id = c0 + threadIdx.x; id < c1; id += FF_BUILD_THREADS) atomicAdd(&s_hist[cell_level[id]], 1);
+    for (int id = id0; id < n_cells; id += stride)
+        if (o == 0) atomicAdd(&s_hist[cell_level[id]], 1);
     __syncthreads();
     if (threadIdx.x < FF_MAX_LEVEL && s_hist[threadIdx.x])
         s_cur[threadIdx.x] += atomicAdd(&g->level_cursor[threadIdx.x], s_hist[threadIdx.x]);
     __syncthreads();
-    const int o = threadIdx.x & 7;
-    const unsigned gmask = 0xffu << (threadIdx.x & 24);
-    for (int id = c0 + (threadIdx.x >> 3); id < c1; id += FF_BUILD_THREADS / 8) {
-        const int first = cell_first[id], l = cell_level[id];
-        const uint32_t k = __ldg(key + first);
-        const int sh = 3 * (FF_MAX_LEVEL - l);             // bits below the level-l prefix
-        const int csh = sh - 3;
-        const uint32_t cpre = (k >> sh) << 3;              // child prefix without the octant
-        // end of octant o = first key >= (cpre + o + 1) << csh; for o = 7 that is the end of the cell
-        // (no overflow: 30-bit keys, the largest bound is 1 << 30)
-        const int e = ff_gallop_bound(key, first, n, (cpre + (uint32_t)o + 1u) << csh);
-        int b = __shfl_up_sync(gmask, e, 1, 8);
-        if (o == 0) b = first;
-        const int cc = e - b;
-        int32_t ent;
-        if (cc == 0) ent = FF_CHILD_EMPTY;
-        else if (cc > nleaf && l + 1 < FF_MAX_LEVEL) ent = cell_base[b] + (l - ff_lprev(key, b));   // internal child: level l+1 at slot b
-        else if (cc == 1) ent = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)b);
-        else { ent = (int32_t)(FF_CHILD_LEAF1 | FF_CHILD_MULTI | (uint32_t)b); leaf_count[b] = cc; }
-        // the eight links are stored COMPACTED: the non-empty sub-cells first, in octant order, then the empty ones
-        // (the walk pushes the first n_children links without looking at them; the moments add them in this order)
-        const int gsh = threadIdx.x & 24;
-        const unsigned present = (__ballot_sync(gmask, cc != 0) >> gsh) & 0xffu;
-        const int nch = __popc(present);
-        const int rank = __popc(present & ((1u << o) - 1u));
-        cell_child[8 * (size_t)id + (cc != 0 ? rank : nch + (o - rank))] = ent;
-        if (o == 7) { cell_end[id] = e; cell_info[id] = make_int4(first, e, nch, l); }
-        if (o == 0) cell_list[atomicAdd(&s_cur[l], 1)] = id;
+    constexpr int U = FF_BUILD_CELLS, R = FF_BUILD_WINDOW / 8;
+    for (int base_id = id0; base_id < n_cells; base_id += U * stride) {
+        int first[U], l[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int id = base_id + u * stride;
+            first[u] = id < n_cells ? cell_first[id] : 0;
+            l[u] = id < n_cells ? cell_level[id] : 0;
+        }
+        // the windows: lane o holds the keys of slots first + o + 8 r; slots past the end count as "beyond the cell"
+        uint32_t kw[U][R];
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int i = first[u] + o + 8 * r;
+                kw[u][r] = (base_id + u * stride < n_cells && i < n) ? __ldg(key + i) : 0xffffffffu;
+            }
+        int e[U], b[U];
+        int32_t ent[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int sh = 3 * (FF_MAX_LEVEL - l[u]);      // bits below the level-l prefix
+            const int csh = sh - 3;
+            const uint32_t k = __shfl_sync(gmask, kw[u][0], 0, 8);
+            const uint32_t pre = k >> sh;
+            // byte o' of (lo, hi) = number of this lane's window keys whose octant inside the cell is <= o'
+            uint32_t lo = 0, hi = 0;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const bool inside = (kw[u][r] >> sh) == pre;
+                const uint32_t c = (kw[u][r] >> csh) & 7u;
+                if (inside) {
+                    if (c < 4u) { lo += 0x01010101u << (8u * c); hi += 0x01010101u; }
+                    else hi += 0x01010101u << (8u * (c - 4u));
+                }
+            }
+#pragma unroll
+            for (int d = 1; d < 8; d <<= 1) {
+                lo += __shfl_xor_sync(gmask, lo, d, 8);
+                hi += __shfl_xor_sync(gmask, hi, d, 8);
+            }
+            const int below = (int)(((o < 4 ? lo : hi) >> (8 * (o & 3))) & 0xffu);   // window keys in octants <= o
+            e[u] = first[u] + below;
+            // every window key lies in octants <= o: the end of octant o is beyond the window
+            // (no overflow in the bound: 30-bit keys, the largest bound is 1 << 30)
+            if (below == FF_BUILD_WINDOW)
+                e[u] = ff_gallop_bound(key, first[u] + FF_BUILD_WINDOW, n, ((pre << 3) + (uint32_t)o + 1u) << csh);
+            b[u] = __shfl_up_sync(gmask, e[u], 1, 8);
+            if (o == 0) b[u] = first[u];
+            // an internal child = the level l+1 cell that starts at slot b.  Cells that start at the same slot are
+            // numbered consecutively by level, so a child starting at this cell's own first slot is id + 1; any other
+            // child is the first cell starting at its slot (L(b) = l there): cell_base[b]
+            const bool internal = e[u] - b[u] > nleaf && l[u] + 1 < FF_MAX_LEVEL;
+            ent[u] = (internal && b[u] != first[u]) ? cell_base[b[u]] : base_id + u * stride + 1;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int id = base_id + u * stride;
+            if (id >= n_cells) break;
+            const int cc = e[u] - b[u];
+            const bool internal = cc > nleaf && l[u] + 1 < FF_MAX_LEVEL;
+            int32_t en = ent[u];
+            if (cc == 0) en = FF_CHILD_EMPTY;
+            else if (internal) ;
+            else if (cc == 1) en = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)b[u]);
+            else { en = (int32_t)(FF_CHILD_LEAF1 | FF_CHILD_MULTI | (uint32_t)b[u]); leaf_count[b[u]] = cc; }
+            // the eight links are stored COMPACTED: the non-empty sub-cells first, in octant order, then the empty ones
+            // (the walk pushes the first n_children links without looking at them; the moments add them in this order)
+            const unsigned present = (__ballot_sync(gmask, cc != 0) >> gsh) & 0xffu;
+            const int nch = __popc(present);
+            const int rank = __popc(present & ((1u << o) - 1u));
+            cell_child[8 * (size_t)id + (cc != 0 ? rank : nch + (o - rank))] = en;
+            if (o == 7) { cell_end[id] = e[u]; cell_info[id] = make_int4(first[u], e[u], nch, l[u]); }
+            if (o == 0) cell_list[atomicAdd(&s_cur[l[u]], 1)] = id;
+        }
     }
+#ifdef FF_BUILD_PROFILE
+    grid.sync();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tq[3]));
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        printf("build phases ns: p1 %llu p2 %llu p3 %llu (n_cells %d)\n", tq[1] - tq[0], tq[2] - tq[1], tq[3] - tq[2], g->n_cells);
+#endif
 }
 
 // ---- a5: Eq. 14: ONE cooperative launch -----------------------
@@ -369,8 +452,9 @@ int ff_launch_build(ff_ctx* c)
         FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_build, FF_BUILD_THREADS, 0));
         if (per_sm < 1) return FF_ERR_CUDA;
     }
-    int tiles = (n + FF_BUILD_TILE - 1) / FF_BUILD_TILE;
-    int blocks = min(tiles, c->num_sms * min(per_sm, 8));
+    // phase 3 is latency bound and wants every thread slot of the GPU; a small n gets as many blocks as it has
+    // groups of 32 particles (a block with no tile skips phases 1-2)
+    int blocks = max(1, min(min((n + 31) / 32, c->num_sms * min(per_sm, 8)), FF_BUILD_MAX_BLOCKS));
     int nleaf = c->nleaf, cap = (int)c->cell_cap;
     void* args[] = { (void*)&c->key[0], (void*)&n, (void*)&nleaf, (void*)&c->scan_blk, (void*)&c->cell_base,
                      (void*)&c->cell_first, (void*)&c->cell_end, (void*)&c->cell_level, (void*)&c->cell_child,

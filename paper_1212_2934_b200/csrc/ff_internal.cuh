@@ -25,6 +25,7 @@
 #define FF_SCAN_THREADS 256
 #define FF_SCAN_ITEMS 8
 #define FF_SCAN_TILE (FF_SCAN_THREADS * FF_SCAN_ITEMS)
+#define FF_BUILD_MAX_BLOCKS 4096     // grid limit of ff_k_build (its per-block counts live in scan_blk)
 
 // ---- walk geometry (ff_walk.cu) ---------------------------------------------
 #ifndef FF_WALK_WARPS
@@ -72,6 +73,8 @@ struct ff_ctx {
     int count_enabled;
     int timing_enabled;
     int tree_built;
+    int globals_clean;        // the device-side build state (bbox, sort tickets, digit histograms) is reset: set by a
+                              // completed ff_build_tree (ff_k_build resets it for the next one), cleared while one runs
     const float* tree_pos;    // the pos array the current tree was built from (ff_eval_bh checks it is given the same one)
     int moments_valid;
     int device;
@@ -181,6 +184,17 @@ __device__ __forceinline__ float ff_ord2f(uint32_t o)
     return __uint_as_float((o & 0x80000000u) ? (o & 0x7fffffffu) : ~o);
 }
 __device__ __forceinline__ int ff_lane() { return threadIdx.x & 31; }
+
+// the device-side state a tree build starts from (thread t of nt): empty bounding box, sort tickets and digit
+// histograms at zero.  Run by ff_k_reset, and by ff_k_build for the NEXT build once the current one has consumed them.
+__device__ __forceinline__ void ff_reset_globals(ff_globals* g, int t, int nt)
+{
+    if (t < 3) { g->bbox_ord[t] = 0xffffffffu; g->bbox_ord[4 + t] = 0u; }
+    if (t < 4) g->counters[t] = 0ull;
+    if (t < FF_SORT_PASSES) g->sort_ticket[t] = 0;
+    if (t < FF_MAX_LEVEL) { g->level_count[t] = 0; g->level_cursor[t] = 0; }
+    for (int i = t; i < FF_SORT_PASSES * FF_RADIX; i += nt) (&g->digit_hist[0][0])[i] = 0u;
+}
 
 // number of leading octant digits two 30-bit keys share (10 if equal)
 __device__ __forceinline__ int ff_common_levels(uint32_t a, uint32_t b)

@@ -9,15 +9,12 @@
 #include "ff_internal.cuh"
 
 // ------------------------------------------------------------------ a1 bbox --
+// Only after ff_create and after a call that failed half way: a completed build leaves this state behind itself
+// (ff_k_build, phase 1).
 __global__ void ff_k_reset(ff_globals* g)
 {
-    int t = threadIdx.x;
-    if (t < 3) { g->bbox_ord[t] = 0xffffffffu; g->bbox_ord[4 + t] = 0u; }
-    if (t < 4) g->counters[t] = 0ull;
-    if (t == 0) { g->n_cells = 0; g->max_level = 0; }
-    if (t < FF_MAX_LEVEL) { g->level_count[t] = 0; g->level_cursor[t] = 0; }
-    if (t < FF_SORT_PASSES) g->sort_ticket[t] = 0;
-    (&g->digit_hist[0][0])[t] = 0u;                        // launched with FF_SORT_PASSES * FF_RADIX threads
+    ff_reset_globals(g, threadIdx.x, blockDim.x);
+    if (threadIdx.x == 0) g->n_cells = 0;
 }
 
 __global__ void __launch_bounds__(256) ff_k_bbox(const float* __restrict__ pos, int n, ff_globals* g)
@@ -252,7 +249,8 @@ int ff_launch_bbox_keys(ff_ctx* c, const float* pos)
 {
     int n = (int)c->n;
     int n_tiles = (n + FF_SORT_TILE - 1) / FF_SORT_TILE;
-    FF_LAUNCH(c, ff_k_reset, 1, FF_SORT_PASSES * FF_RADIX, 0, c->g);
+    if (!c->globals_clean) FF_LAUNCH(c, ff_k_reset, 1, 256, 0, c->g);
+    c->globals_clean = 0;                                  // until ff_k_build has been enqueued
     int blocks = min((n + 255) / 256, c->num_sms * 8);
     FF_LAUNCH(c, ff_k_bbox, blocks, 256, 0, pos, n, c->g);
     // every block ends with 1024 global atomics (its digit histograms): few blocks while the launch is latency
