@@ -55,7 +55,8 @@ ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n,
     tg.ux = ff_pin_pair(__ldg(mom + o0), __ldg(mom + o1));
     tg.uy = ff_pin_pair(__ldg(mom + o0 + 1), __ldg(mom + o1 + 1));
     tg.uz = ff_pin_pair(__ldg(mom + o0 + 2), __ldg(mom + o1 + 2));
-    double acc0[7] = { 0, 0, 0, 0, 0, 0, 0 }, acc1[7] = { 0, 0, 0, 0, 0, 0, 0 };
+    // fp64 running sums per target: h (3), T_aa (3), G_ab (3) of the tensor form (ff_pair.cuh), f^sr (3, LJ only)
+    double acc0[12] = { 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0 }, acc1[12] = { 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0 };
     const int n_tiles = (n + FF_DIRECT_THREADS - 1) / FF_DIRECT_THREADS;
     for (int tile = blockIdx.y; tile < n_tiles; tile += splits) {
         const int j = tile * FF_DIRECT_THREADS + t;
@@ -74,8 +75,9 @@ ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n,
         const bool own = (tile >> 1) == (int)blockIdx.x;
         const bool own_second = tile & 1;
         for (int c0 = 0; c0 < FF_DIRECT_THREADS; c0 += 32) {
-            ff_acc2 s;
-            ff_acc2_zero(s);
+            ff_accg2 s;
+            ff_accg2_zero(s);
+            float2 lx = ff_dup(0.0f), ly = lx, lz = lx;     // LJ: sum_j w rho
             if (own) {
 #pragma unroll 2
                 for (int i = 0; i < 32; ++i) {
@@ -87,8 +89,11 @@ ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n,
                     if (c0 + i == t) {                     // j != k (Alg. 1 line 5): r2 = 0 gave inf, dropped here
                         if (own_second) rinv.y = 0.0f; else rinv.x = 0.0f;
                     }
-                    if (LJ) ff_pair2_accum<true>(A, B, tg, dx, dy, dz, rinv, s, ff_lj2(r2, rinv, lj));
-                    else ff_pair2_accum(A, B, tg, dx, dy, dz, rinv, s);
+                    ff_pair2g_accum(A, B, dx, dy, dz, rinv, s);
+                    if (LJ) {
+                        const float2 w = ff_lj2(r2, rinv, lj);
+                        lx = __ffma2_rn(w, dx, lx); ly = __ffma2_rn(w, dy, ly); lz = __ffma2_rn(w, dz, lz);
+                    }
                 }
             } else {
 #pragma unroll 4
@@ -99,21 +104,33 @@ ff_k_direct(const float* __restrict__ pos, const float* __restrict__ mom, int n,
                         float2 dx, dy, dz, r2;
                         ff_pair2_geom(A, tg, dx, dy, dz, r2);
                         const float2 rinv = ff_rsqrt2(r2);
-                        ff_pair2_accum<true>(A, B, tg, dx, dy, dz, rinv, s, ff_lj2(r2, rinv, lj));
+                        ff_pair2g_accum(A, B, dx, dy, dz, rinv, s);
+                        const float2 w = ff_lj2(r2, rinv, lj);
+                        lx = __ffma2_rn(w, dx, lx); ly = __ffma2_rn(w, dy, ly); lz = __ffma2_rn(w, dz, lz);
                     } else {
-                        ff_pair2(A, B, tg, s);
+                        ff_pair2g(A, B, tg, s);
                     }
                 }
             }
-            acc0[0] += s.hx.x; acc0[1] += s.hy.x; acc0[2] += s.hz.x; acc0[3] += s.fx.x; acc0[4] += s.fy.x;
-            acc0[5] += s.fz.x; acc0[6] += s.sk.x;
-            acc1[0] += s.hx.y; acc1[1] += s.hy.y; acc1[2] += s.hz.y; acc1[3] += s.fx.y; acc1[4] += s.fy.y;
-            acc1[5] += s.fz.y; acc1[6] += s.sk.y;
+            acc0[0] += s.hx.x; acc0[1] += s.hy.x; acc0[2] += s.hz.x; acc0[3] += s.txx.x; acc0[4] += s.tyy.x;
+            acc0[5] += s.tzz.x; acc0[6] += s.gxy.x; acc0[7] += s.gxz.x; acc0[8] += s.gyz.x;
+            acc1[0] += s.hx.y; acc1[1] += s.hy.y; acc1[2] += s.hz.y; acc1[3] += s.txx.y; acc1[4] += s.tyy.y;
+            acc1[5] += s.tzz.y; acc1[6] += s.gxy.y; acc1[7] += s.gxz.y; acc1[8] += s.gyz.y;
+            if (LJ) {
+                acc0[9] += lx.x; acc0[10] += ly.x; acc0[11] += lz.x;
+                acc1[9] += lx.y; acc1[10] += ly.y; acc1[11] += lz.y;
+            }
         }
     }
     auto finish = [&](int k, double* acc, float ux, float uy, float uz) {
         if (k >= n) return;
-        acc[3] += acc[6] * (double)ux; acc[4] += acc[6] * (double)uy; acc[5] += acc[6] * (double)uz;
+        // f = G u_k (+ f^sr): G_aa = 2 T_aa + S, S = sum_j p a = -(2/3) tr T (the tensor is traceless term by term)
+        const double S = -(2.0 / 3.0) * (acc[3] + acc[4] + acc[5]);
+        const double gxx = 2.0 * acc[3] + S, gyy = 2.0 * acc[4] + S, gzz = 2.0 * acc[5] + S;
+        const double fx = gxx * ux + acc[6] * uy + acc[7] * uz + acc[9];
+        const double fy = acc[6] * ux + gyy * uy + acc[8] * uz + acc[10];
+        const double fz = acc[7] * ux + acc[8] * uy + gzz * uz + acc[11];
+        acc[3] = fx; acc[4] = fy; acc[5] = fz;
         if (splits == 1) {
             if (H_out) { H_out[3 * (size_t)k] = (float)acc[0]; H_out[3 * (size_t)k + 1] = (float)acc[1]; H_out[3 * (size_t)k + 2] = (float)acc[2]; }
             if (F_out) { F_out[3 * (size_t)k] = (float)acc[3]; F_out[3 * (size_t)k + 1] = (float)acc[4]; F_out[3 * (size_t)k + 2] = (float)acc[5]; }

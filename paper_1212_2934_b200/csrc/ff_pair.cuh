@@ -69,11 +69,10 @@ __device__ __forceinline__ void ff_pair2_geom(const float4& A, const ff_target2&
 //   h_kj = 3 rho (u_j.rho)/r^5 - u_j/r^3
 //   f_kj = { rho [(u_j.u_k) - 5 (u_j.rho)(u_k.rho)/r^2] + u_k (u_j.rho) + u_j (u_k.rho) } 3/r^5
 // 38 packed FP32 instructions + 2 MUFU.RSQ per source and target pair (ff_pair2_geom included).
-// EXTRA: `extra` is added to the coefficient of rho in f (the all-pairs MD step puts the Lennard-Jones term of
-// Eq. 13 there: f^sr_kj = w rho with w = 24 eps [ (s/r)^12 - (s/r)^6 ] / r^2, PAPER.md:74 and Algorithm 1 line 8)
-template <bool EXTRA = false>
+// (the vector form: used with the first-order cell term below, which needs u_k.rho anyway; the walk's and the
+// all-pairs kernel's main loops use the tensor form further down)
 __device__ __forceinline__ void ff_pair2_accum(const float4& A, const float2& B, const ff_target2& t, float2 dx, float2 dy,
-                                               float2 dz, float2 rinv, ff_acc2& s, float2 extra = make_float2(0.f, 0.f))
+                                               float2 dz, float2 rinv, ff_acc2& s)
 {
     const float2 mx = ff_dup(A.w), my = ff_dup(B.x), mz = ff_dup(B.y);
     const float2 rinv2 = __fmul2_rn(rinv, rinv);
@@ -87,11 +86,65 @@ __device__ __forceinline__ void ff_pair2_accum(const float4& A, const float2& B,
     s.hx = __ffma2_rn(ca, dx, s.hx); s.hy = __ffma2_rn(ca, dy, s.hy); s.hz = __ffma2_rn(ca, dz, s.hz);
     s.hx = __ffma2_rn(nr3, mx, s.hx); s.hy = __ffma2_rn(nr3, my, s.hy); s.hz = __ffma2_rn(nr3, mz, s.hz);
     const float2 w = __fmul2_rn(__fmul2_rn(ca, b), rinv2);                         // 3 (u_j.rho)(u_k.rho) / r^7
-    float2 cr = __ffma2_rn(ff_dup(-5.0f), w, __fmul2_rn(c, r5));
-    if (EXTRA) cr = __fadd2_rn(cr, extra);
+    const float2 cr = __ffma2_rn(ff_dup(-5.0f), w, __fmul2_rn(c, r5));
     s.fx = __ffma2_rn(cr, dx, s.fx); s.fy = __ffma2_rn(cr, dy, s.fy); s.fz = __ffma2_rn(cr, dz, s.fz);
     s.fx = __ffma2_rn(cb, mx, s.fx); s.fy = __ffma2_rn(cb, my, s.fy); s.fz = __ffma2_rn(cb, mz, s.fz);
     s.sk = __fadd2_rn(s.sk, ca);
+}
+
+
+// ---- the same pair terms with the force kept as a TENSOR ---------------------------------------------------------
+// Eq. 12 is linear in the target's moment: f_k = G u_k with the symmetric, traceless field-gradient tensor
+//     G = sum_j { p (rho (x) u_j + u_j (x) rho + a 1) + q rho (x) rho },   p = 3/r^5, a = u_j.rho, q = -5 p a / r^2
+//       = sum_j { (p rho) (x) e + e (x) (p rho) + p a 1 },                 e = u_j - 2.5 (a / r^2) rho
+// so the target's moment leaves the loop: no u_k.rho, no u_j.u_k, and the nine sums h (3), T_aa = sum (p rho_a) e_a (3),
+// G_ab (3 off-diagonal) are applied to u_k once at the end.  The diagonal needs no sum of its own: the tensor is
+// traceless term by term (rho.e = -1.5 a), so sum_j p a = -(2/3)(Txx + Tyy + Tzz).
+// 36 packed FP32 instructions + 2 MUFU.RSQ per source and target pair (38 with the vector form above).
+struct ff_accg2 {
+    float2 hx, hy, hz, txx, tyy, tzz, gxy, gxz, gyz;
+};
+__device__ __forceinline__ void ff_accg2_zero(ff_accg2& s)
+{
+    s.hx = s.hy = s.hz = s.txx = s.tyy = s.tzz = s.gxy = s.gxz = s.gyz = ff_dup(0.0f);
+}
+
+__device__ __forceinline__ void ff_pair2g_accum(const float4& A, const float2& B, float2 dx, float2 dy, float2 dz,
+                                                float2 rinv, ff_accg2& s)
+{
+    const float2 mx = ff_dup(A.w), my = ff_dup(B.x), mz = ff_dup(B.y);
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 nr3 = __fmul2_rn(rinv2, make_float2(-rinv.x, -rinv.y));           // -1 / r^3
+    const float2 p = __fmul2_rn(nr3, __fmul2_rn(rinv2, ff_dup(-3.0f)));            // 3 / r^5
+    const float2 a = __ffma2_rn(mz, dz, __ffma2_rn(my, dy, __fmul2_rn(mx, dx)));   // u_j . rho
+    const float2 px = __fmul2_rn(p, dx), py = __fmul2_rn(p, dy), pz = __fmul2_rn(p, dz);   // p rho
+    s.hx = __ffma2_rn(px, a, s.hx); s.hy = __ffma2_rn(py, a, s.hy); s.hz = __ffma2_rn(pz, a, s.hz);
+    s.hx = __ffma2_rn(nr3, mx, s.hx); s.hy = __ffma2_rn(nr3, my, s.hy); s.hz = __ffma2_rn(nr3, mz, s.hz);
+    const float2 m = __fmul2_rn(a, __fmul2_rn(rinv2, ff_dup(-2.5f)));              // -2.5 a / r^2
+    const float2 ex = __ffma2_rn(m, dx, mx), ey = __ffma2_rn(m, dy, my), ez = __ffma2_rn(m, dz, mz);
+    s.txx = __ffma2_rn(px, ex, s.txx); s.tyy = __ffma2_rn(py, ey, s.tyy); s.tzz = __ffma2_rn(pz, ez, s.tzz);
+    s.gxy = __ffma2_rn(px, ey, s.gxy); s.gxy = __ffma2_rn(py, ex, s.gxy);
+    s.gxz = __ffma2_rn(px, ez, s.gxz); s.gxz = __ffma2_rn(pz, ex, s.gxz);
+    s.gyz = __ffma2_rn(py, ez, s.gyz); s.gyz = __ffma2_rn(pz, ey, s.gyz);
+}
+
+// f = G u for the lane's two targets: G_aa = 2 T_aa + S with S = sum_j p a = -(2/3) tr T, off-diagonals as summed
+__device__ __forceinline__ void ff_accg2_apply(const ff_accg2& s, float2 ux, float2 uy, float2 uz, float2& fx, float2& fy,
+                                               float2& fz)
+{
+    const float2 S = __fmul2_rn(__fadd2_rn(__fadd2_rn(s.txx, s.tyy), s.tzz), ff_dup(-2.0f / 3.0f));
+    const float2 two = ff_dup(2.0f);
+    const float2 gxx = __ffma2_rn(two, s.txx, S), gyy = __ffma2_rn(two, s.tyy, S), gzz = __ffma2_rn(two, s.tzz, S);
+    fx = __ffma2_rn(s.gxz, uz, __ffma2_rn(s.gxy, uy, __fmul2_rn(gxx, ux)));
+    fy = __ffma2_rn(s.gyz, uz, __ffma2_rn(gyy, uy, __fmul2_rn(s.gxy, ux)));
+    fz = __ffma2_rn(gzz, uz, __ffma2_rn(s.gyz, uy, __fmul2_rn(s.gxz, ux)));
+}
+
+__device__ __forceinline__ void ff_pair2g(const float4& A, const float2& B, const ff_target2& t, ff_accg2& s)
+{
+    float2 dx, dy, dz, r2;
+    ff_pair2_geom(A, t, dx, dy, dz, r2);
+    ff_pair2g_accum(A, B, dx, dy, dz, ff_rsqrt2(r2), s);
 }
 
 // ---- first-order cell term (FF_OPT_CELL_ORDER = 1) -------------------------
@@ -142,12 +195,4 @@ __device__ __forceinline__ void ff_pair2_quad(const float4& A, const float2& B, 
     s.sk = __fadd2_rn(s.sk, e);
     sq.gxx = __ffma2_rn(c1, Dxx, sq.gxx); sq.gyy = __ffma2_rn(c1, Dyy, sq.gyy); sq.gzz = __ffma2_rn(c1, Dzz, sq.gzz);
     sq.gxy = __ffma2_rn(c1, Dxy, sq.gxy); sq.gxz = __ffma2_rn(c1, Dxz, sq.gxz); sq.gyz = __ffma2_rn(c1, Dyz, sq.gyz);
-}
-
-// one source against the lane's two targets, nothing masked (the hot loop of the walk and of the direct kernel)
-__device__ __forceinline__ void ff_pair2(const float4& A, const float2& B, const ff_target2& t, ff_acc2& s)
-{
-    float2 dx, dy, dz, r2;
-    ff_pair2_geom(A, t, dx, dy, dz, r2);
-    ff_pair2_accum(A, B, t, dx, dy, dz, ff_rsqrt2(r2), s);
 }

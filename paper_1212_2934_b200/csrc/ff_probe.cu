@@ -79,17 +79,17 @@ ff_k_probe_eval(int iters, float seed, float* __restrict__ sink)
     tg.px = make_float2(b, b + 6.f); tg.py = make_float2(b * 0.5f + 1.f, b * 0.5f + 4.f); tg.pz = make_float2(2.f - b, -4.f - b);
     tg.ux = make_float2(0.6f + 1e-3f * lane, 0.8f - 1e-3f * lane); tg.uy = make_float2(1e-3f * lane, -1e-3f * lane);
     tg.uz = make_float2(0.8f, 0.6f);
-    ff_acc2 s;
-    ff_acc2_zero(s);
+    ff_accg2 s;
+    ff_accg2_zero(s);
     for (int it = 0; it < iters; ++it) {
         const float4* pa = qa[w] + half;
         const float2* pb = qb[w] + half;
 #pragma unroll 4
-        for (int i = 0; i < 16; ++i) ff_pair2(pa[2 * i], pb[2 * i], tg, s);
+        for (int i = 0; i < 16; ++i) ff_pair2g(pa[2 * i], pb[2 * i], tg, s);
         __syncwarp();
     }
-    const float r = s.hx.x + s.hx.y + s.hy.x + s.hy.y + s.hz.x + s.hz.y + s.fx.x + s.fx.y + s.fy.x + s.fy.y + s.fz.x +
-                    s.fz.y + s.sk.x + s.sk.y;
+    const float r = s.hx.x + s.hx.y + s.hy.x + s.hy.y + s.hz.x + s.hz.y + s.txx.x + s.txx.y + s.tyy.x + s.tyy.y + s.tzz.x +
+                    s.tzz.y + s.gxy.x + s.gxy.y + s.gxz.x + s.gxz.y + s.gyz.x + s.gyz.y;
     if (r == 12345.678f) sink[0] = r;
 }
 

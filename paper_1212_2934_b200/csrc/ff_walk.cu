@@ -128,10 +128,12 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
         tg.px = make_float2(xy.x, xy.y); tg.py = make_float2(xy.z, xy.w); tg.pz = sm.mem_z[ti];
         tg.ux = make_float2(uxy.x, uxy.y); tg.uy = make_float2(uxy.z, uxy.w); tg.uz = sm.mem_uz[ti];
     }
-    ff_acc2 s;
+    ff_acc2 s;                                             // QUAD: vector form of the force + cell-tensor sums
     ff_acc2_zero(s);
     ff_accq2 sq;
     ff_accq2_zero(sq);
+    ff_accg2 sg;                                           // otherwise: field + force-gradient tensor (ff_pair.cuh)
+    ff_accg2_zero(sg);
     __syncwarp();
     // the group's own members: direct terms, self skipped by index (Alg. 1 line 5);
     // slots >= nm of a ragged last group hold copies of the last member and are masked the same way
@@ -145,7 +147,8 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
         float2 rinv;
         rinv.x = (j == i0 || j >= nm) ? 0.0f : ff_rsqrt(r2.x);
         rinv.y = (j == i1 || j >= nm) ? 0.0f : ff_rsqrt(r2.y);
-        ff_pair2_accum(A, B, tg, dx, dy, dz, rinv, s);
+        if (QUAD) ff_pair2_accum(A, B, tg, dx, dy, dz, rinv, s);
+        else ff_pair2g_accum(A, B, dx, dy, dz, rinv, sg);
     }
     if (COUNT) c_part += (unsigned long long)nm * (unsigned long long)(nm - 1);
     __syncwarp();
@@ -170,9 +173,9 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
             }
         } else if (iters == BATCH_ITERS) {
 #pragma unroll 4
-            for (int i = 0; i < BATCH_ITERS; ++i) ff_pair2(qa[ST * i], qb[ST * i], tg, s);
+            for (int i = 0; i < BATCH_ITERS; ++i) ff_pair2g(qa[ST * i], qb[ST * i], tg, sg);
         } else {
-            for (int i = 0; i < iters; ++i) ff_pair2(qa[ST * i], qb[ST * i], tg, s);
+            for (int i = 0; i < iters; ++i) ff_pair2g(qa[ST * i], qb[ST * i], tg, sg);
         }
         __syncwarp();
     };
@@ -388,7 +391,11 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
     // W = 32: lanes l and l + 16 hold partial sums of the same two targets
     if (W == 32) {
 #define FF_FOLD(v) v.x += __shfl_xor_sync(FF_FULL, v.x, 16); v.y += __shfl_xor_sync(FF_FULL, v.y, 16)
-        FF_FOLD(s.hx); FF_FOLD(s.hy); FF_FOLD(s.hz); FF_FOLD(s.fx); FF_FOLD(s.fy); FF_FOLD(s.fz); FF_FOLD(s.sk);
+        if (QUAD) { FF_FOLD(s.hx); FF_FOLD(s.hy); FF_FOLD(s.hz); FF_FOLD(s.fx); FF_FOLD(s.fy); FF_FOLD(s.fz); FF_FOLD(s.sk); }
+        else {
+            FF_FOLD(sg.hx); FF_FOLD(sg.hy); FF_FOLD(sg.hz); FF_FOLD(sg.txx); FF_FOLD(sg.tyy); FF_FOLD(sg.tzz);
+            FF_FOLD(sg.gxy); FF_FOLD(sg.gxz); FF_FOLD(sg.gyz);
+        }
         if (QUAD) { FF_FOLD(sq.gxx); FF_FOLD(sq.gyy); FF_FOLD(sq.gzz); FF_FOLD(sq.gxy); FF_FOLD(sq.gxz); FF_FOLD(sq.gyz); }
 #undef FF_FOLD
     }
@@ -399,6 +406,12 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
         const float2 gy = __ffma2_rn(sq.gyz, tg.uz, __ffma2_rn(sq.gyy, tg.uy, __fmul2_rn(sq.gxy, tg.ux)));
         const float2 gz = __ffma2_rn(sq.gzz, tg.uz, __ffma2_rn(sq.gyz, tg.uy, __fmul2_rn(sq.gxz, tg.ux)));
         s.fx = __ffma2_rn(m2, gx, s.fx); s.fy = __ffma2_rn(m2, gy, s.fy); s.fz = __ffma2_rn(m2, gz, s.fz);
+    }
+    if (!QUAD) {
+        // f_k = G u_k (Eq. 12 is linear in u_k); the result goes where the vector form keeps it
+        ff_accg2_apply(sg, tg.ux, tg.uy, tg.uz, s.fx, s.fy, s.fz);
+        s.hx = sg.hx; s.hy = sg.hy; s.hz = sg.hz;
+        s.sk = ff_dup(0.0f);
     }
     // (the moments are read back from the packed target registers: keeping the loaded float4 alive across the
     // walk makes ptxas rebuild the register pairs with MOVs inside the evaluation loop)
