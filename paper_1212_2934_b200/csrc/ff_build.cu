@@ -18,11 +18,11 @@
 namespace cg = cooperative_groups;
 
 #ifndef FF_MOM_THREADS
-#define FF_MOM_THREADS 256
+#define FF_MOM_THREADS 512
 #endif
 #define FF_MOM_SOLO 1                 // levels 0..1 of the moment pass run in one block
 #ifndef FF_BUILD_THREADS
-#define FF_BUILD_THREADS 256
+#define FF_BUILD_THREADS 512
 #endif
 #define FF_BUILD_ITEMS 8
 #define FF_BUILD_TILE (FF_BUILD_THREADS * FF_BUILD_ITEMS)

@@ -35,7 +35,10 @@
 #define FF_WALK_MINB 5             // min resident blocks per SM asked of ptxas (caps registers at 96; 5 x 4 warps per SM)
 #endif
 #define FF_WALK_STACK 1024         // traversal stack entries per warp
-#define FF_WALK_PEND 64            // pending interaction ring per warp (two batches of 32)
+#ifndef FF_WALK_BATCH
+#define FF_WALK_BATCH 64           // ring entries evaluated in one go
+#endif
+#define FF_WALK_PEND (2 * FF_WALK_BATCH)   // pending interaction ring per warp (two batches)
 #ifndef FF_WALK_PROBE_PAIRS
 #define FF_WALK_PROBE_PAIRS 2      // probe members (x2) of the opening pre-filter: the members at the x and y extremes
 #endif                             // of the group's box

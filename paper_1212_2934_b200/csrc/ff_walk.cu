@@ -60,7 +60,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
           float* __restrict__ F_out, unsigned long long* __restrict__ counters)
 {
     constexpr int ST = (W == 32) ? 2 : 1;                  // ring entries per evaluation step of one lane
-    constexpr int BATCH_ITERS = 32 / ST;                   // evaluation steps per batch of 32 ring entries
+    constexpr int BATCH_ITERS = FF_WALK_BATCH / ST;        // evaluation steps per batch of ring entries
     const int g0 = grp * W;
     const int g1 = min(n, g0 + W);
     const int nm = g1 - g0;
@@ -154,7 +154,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
     __syncwarp();
 
     const float th2 = __fmul_rn(theta, theta);
-    int pend_head = 0, pend_cnt = 0;                       // warp-uniform ring state (entries); head is 0 or 32
+    int pend_head = 0, pend_cnt = 0;                       // warp-uniform ring state (entries); head is 0 or FF_WALK_BATCH
     int sp_top = 0;                                        // warp-uniform stack size
 
     // evaluate `iters` steps of this lane starting at ring entry pend_head (W = 32: entries head + 2 i + half)
@@ -191,10 +191,10 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
         pend_cnt += __popc(m);
     };
     auto drain = [&]() {
-        while (pend_cnt >= 32) {
+        while (pend_cnt >= FF_WALK_BATCH) {
             eval(BATCH_ITERS);
-            pend_head ^= 32;
-            pend_cnt -= 32;
+            pend_head ^= FF_WALK_BATCH;
+            pend_cnt -= FF_WALK_BATCH;
         }
     };
     // a leaf with several particles (depth cap, or N_leaf > 8): the warp streams it through the ring
