@@ -51,7 +51,10 @@ typedef enum ff_status {
     FF_ERR_NO_TREE = -3,        /* ff_eval_bh / ff_get_tree before ff_build_tree */
     FF_ERR_CAPACITY = -4,       /* internal pool overflow (cannot happen with ff_workspace_bytes' sizing; kept for the ABI).
                                    Detected on the device, reported by the next ff_get_tree / ff_get_timings / ff_get_counters */
-    FF_ERR_CUDA = -5            /* CUDA runtime / launch failure; text via ff_last_error */
+    FF_ERR_CUDA = -5,           /* CUDA runtime / launch failure; text via ff_last_error */
+    FF_ERR_CHECK = -6           /* checked build only (library compiled with -DFF_CHECKED): a device-side index or bound
+                                   check failed; reported like FF_ERR_CAPACITY, the failing source line is in
+                                   ff_last_error after the reporting call */
 } ff_status;
 
 #define FF_MAX_N (1ll << 28)    /* particle slots must fit the 30-bit stack entries of the walk */

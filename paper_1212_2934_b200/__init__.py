@@ -21,7 +21,7 @@ from . import build as _build
 _lib = None
 
 FF_OK = 0
-FF_ERR_INVALID_ARG, FF_ERR_WORKSPACE, FF_ERR_NO_TREE, FF_ERR_CAPACITY, FF_ERR_CUDA = -1, -2, -3, -4, -5
+FF_ERR_INVALID_ARG, FF_ERR_WORKSPACE, FF_ERR_NO_TREE, FF_ERR_CAPACITY, FF_ERR_CUDA, FF_ERR_CHECK = -1, -2, -3, -4, -5, -6
 FF_OPT_THETA, FF_OPT_NLEAF, FF_OPT_COUNTERS, FF_OPT_TIMING, FF_OPT_GROUP, FF_OPT_CELL_ORDER = 1, 2, 3, 4, 5, 6
 FF_N_PHASES = 7
 PHASES = ("bbox_keys", "sort", "build", "moments", "walk", "direct", "step")
@@ -77,7 +77,7 @@ def lib():
     """Load libff.so (building it in-tree with nvcc if it is missing or stale).  Raises if that fails."""
     global _lib
     if _lib is None:
-        so = _build.build()
+        so = _build.build(checked=os.environ.get("FF_CHECKED", "0") == "1")
         L = ctypes.CDLL(so)
         vp, i64, i32, f32, f64, u64 = (ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_float,
                                        ctypes.c_double, ctypes.c_uint64)
@@ -179,7 +179,7 @@ class FFContext:
     def _check(self, rc, where):
         if rc != FF_OK:
             detail = ""
-            if rc == FF_ERR_CUDA and getattr(self, "_h", None):
+            if rc in (FF_ERR_CUDA, FF_ERR_CHECK) and getattr(self, "_h", None):
                 detail = self._L.ff_last_error(self._h).decode()
             raise FFError(rc, where, detail)
 

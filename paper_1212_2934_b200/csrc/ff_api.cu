@@ -320,9 +320,10 @@ extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* ang
 // the sticky device-side error flag (FF_ERR_CAPACITY), read at a point where the stream is synchronised
 static int ff_device_error(ff_ctx* c)
 {
-    int32_t err = 0;
-    FF_CUDA(c, cudaMemcpy(&err, &c->g->error, sizeof(err), cudaMemcpyDeviceToHost));
-    return err;
+    int32_t err[2] = { 0, 0 };                             // error, check_line
+    FF_CUDA(c, cudaMemcpy(err, &c->g->error, sizeof(err), cudaMemcpyDeviceToHost));
+    if (err[0] == FF_ERR_CHECK) snprintf(c->last_error, sizeof(c->last_error), "device-side check failed at source line %d", err[1]);
+    return err[0];
 }
 
 extern "C" int ff_get_tree(ff_ctx* c, ff_tree_view* out)
@@ -333,7 +334,7 @@ extern "C" int ff_get_tree(ff_ctx* c, ff_tree_view* out)
     FF_CUDA(c, cudaStreamSynchronize(c->stream));
     ff_globals g;
     FF_CUDA(c, cudaMemcpy(&g, c->g, sizeof(g), cudaMemcpyDeviceToHost));
-    if (g.error) return g.error;
+    if (g.error) return ff_device_error(c);
     memset(out, 0, sizeof(*out));
     out->n = c->n; out->n_cells = g.n_cells; out->nleaf = c->nleaf;
     out->lo[0] = g.lo[0]; out->lo[1] = g.lo[1]; out->lo[2] = g.lo[2]; out->S = g.S;
@@ -415,6 +416,7 @@ extern "C" const char* ff_error_string(int code)
     case FF_ERR_NO_TREE: return "no tree: call ff_build_tree first";
     case FF_ERR_CAPACITY: return "cell pool capacity exceeded";
     case FF_ERR_CUDA: return "CUDA error (see ff_last_error)";
+    case FF_ERR_CHECK: return "device-side check failed (checked build; see ff_last_error)";
     default: return "unknown error code";
     }
 }

@@ -172,6 +172,7 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
                 if (fits)
                     for (uint32_t q = 0; q < c[r]; ++q) {
                         const int l = lp[r] + 1 + (int)q;
+                        FF_CHECK(g, run + q < (uint32_t)cell_cap && l >= 0 && l < FF_MAX_LEVEL);
                         cell_first[run + q] = i;
                         cell_level[run + q] = l;
                         atomicAdd(&s_hist[l], 1);
@@ -282,6 +283,8 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
             const int cc = e[u] - b[u];
             const bool internal = cc > nleaf && l[u] + 1 < FF_MAX_LEVEL;
             int32_t en = ent[u];
+            FF_CHECK(g, first[u] <= b[u] && b[u] <= e[u] && e[u] <= n && (o != 7 || e[u] > first[u]));
+            FF_CHECK(g, !(cc != 0 && internal) || (en > id && en < n_cells));
             if (cc == 0) en = FF_CHILD_EMPTY;
             else if (internal) ;
             else if (cc == 1) en = (int32_t)(FF_CHILD_LEAF1 | (uint32_t)b[u]);
@@ -293,7 +296,11 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
             const int rank = __popc(present & ((1u << o) - 1u));
             cell_child[8 * (size_t)id + (cc != 0 ? rank : nch + (o - rank))] = en;
             if (o == 7) { cell_end[id] = e[u]; cell_info[id] = make_int4(first[u], e[u], nch, l[u]); }
-            if (o == 0) cell_list[atomicAdd(&s_cur[l[u]], 1)] = id;
+            if (o == 0) {
+                const int at = atomicAdd(&s_cur[l[u]], 1);
+                FF_CHECK(g, at >= 0 && at < n_cells);
+                cell_list[at] = id;
+            }
         }
     }
 #ifdef FF_BUILD_PROFILE
@@ -370,6 +377,7 @@ ff_k_moments(const float* __restrict__ mom, const uint32_t* __restrict__ perm, i
         for (int k = k0; k < le; k += kstep) {
             const int id = id1;
             const int32_t e = e1;
+            FF_CHECK(g, id >= 0 && id < g->n_cells && (e < 0 || (e > id && e < g->n_cells)));
             id1 = id2;
             id2 = k + 2 * kstep < le ? cell_list[k + 2 * kstep] : -1;
             e1 = id1 >= 0 ? cell_child[8 * (size_t)id1 + o] : FF_CHILD_EMPTY;

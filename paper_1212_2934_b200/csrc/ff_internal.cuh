@@ -57,6 +57,7 @@ struct ff_globals {
     float inv;                // fl(1024 / S)
     int32_t n_cells;          // internal cells of the current tree
     int32_t error;            // sticky device-side error flag (FF_ERR_*)
+    int32_t check_line;       // FF_CHECKED: source line of the first failed device-side check
     int32_t max_level;        // deepest level holding an internal cell
     int32_t level_count[FF_MAX_LEVEL];      // internal cells per level (ff_k_build)
     int32_t level_cursor[FF_MAX_LEVEL];     // fill cursors of the level lists
@@ -175,6 +176,19 @@ int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n, f
 int ff_launch_probe(ff_ctx* c, int kind, int iters, double* tflops);
 int ff_launch_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n,
                    const ff_step_params* p, uint64_t step_index);
+
+// ---- checked build (-DFF_CHECKED): device-side index and bound checks of every kernel --------------------------
+// compute-sanitizer is not available on every machine this runs on; the checked library is what
+// tests/sanitizer_smoke.py runs against instead.  A failed check sets the sticky error flag (first one wins) and the
+// kernel carries on; the release build compiles the checks away.
+#ifdef FF_CHECKED
+#define FF_CHECK(g, cond)                                                                    \
+    do {                                                                                     \
+        if (!(cond) && atomicCAS(&(g)->error, 0, (int32_t)FF_ERR_CHECK) == 0) (g)->check_line = __LINE__; \
+    } while (0)
+#else
+#define FF_CHECK(g, cond) do { } while (0)
+#endif
 
 // ---- small device helpers --------------------------------------------------------
 __device__ __forceinline__ uint32_t ff_f2ord(float f)

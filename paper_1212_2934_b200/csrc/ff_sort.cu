@@ -91,6 +91,7 @@ __global__ void __launch_bounds__(256) ff_k_keys(const float* __restrict__ pos, 
         for (int a = 0; a < 3; ++a) {
             float d = __fsub_rn(__ldg(pos + 3 * (size_t)i + a), lo[a]);
             int v = __float2int_rd(__fmul_rn(d, inv));      // floor, then to int
+            FF_CHECK(g, v >= 0 && v <= 1024);
             q[a] = (uint32_t)min(1023, max(0, v));
         }
         const uint32_t k = (ff_spread10(q[0]) << 2) | (ff_spread10(q[1]) << 1) | ff_spread10(q[2]);
@@ -145,6 +146,7 @@ ff_k_radix_onesweep(const uint32_t* __restrict__ kin, const uint32_t* __restrict
 #pragma unroll
     for (int k = 0; k < 8; ++k) if (k < w) dbase += wsum[k];
     const int tile = s_tile;
+    FF_CHECK(g, tile >= 0 && tile * FF_SORT_TILE < n);
 
     uint32_t key[FF_SORT_ROUNDS], val[FF_SORT_ROUNDS], rank[FF_SORT_ROUNDS];
     const int base = tile * FF_SORT_TILE + w * 32 * FF_SORT_ROUNDS;
@@ -237,6 +239,7 @@ ff_k_radix_onesweep(const uint32_t* __restrict__ kin, const uint32_t* __restrict
             uint32_t k = skey[i];
             uint32_t dst = tile_base[(k >> shift) & (FF_RADIX - 1)] + (uint32_t)i;
             const uint32_t v = sval[i];
+            FF_CHECK(g, dst < (uint32_t)n && v < (uint32_t)n);
             kout[dst] = k;
             vout[dst] = v;
             // last pass: dst is the final sorted slot, so the sorted float4 positions are written here as well

@@ -91,6 +91,7 @@ ff_k_lj(const uint32_t* __restrict__ key, const float4* __restrict__ pos_s, cons
 #pragma unroll
         for (int d = 0; d < 3; ++d)
             for (int j = b[d]; j < e[d]; ++j) {
+                FF_CHECK(const_cast<ff_globals*>(g), j >= 0 && j < n);
                 const float4 q = __ldg(pos_s + j);
                 const float rx = p.x - q.x, ry = p.y - q.y, rz = p.z - q.z;
                 const float r2 = fmaf(rz, rz, fmaf(ry, ry, rx * rx));

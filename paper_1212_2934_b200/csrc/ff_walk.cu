@@ -57,7 +57,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
           const int4* __restrict__ cell_info, const int4* __restrict__ cell_child,
           const int32_t* __restrict__ leaf_count, const float4* __restrict__ centre,
           const float4* __restrict__ moment, const float4* __restrict__ quad, float* __restrict__ H_out,
-          float* __restrict__ F_out, unsigned long long* __restrict__ counters)
+          float* __restrict__ F_out, unsigned long long* __restrict__ counters, ff_globals* __restrict__ g)
 {
     constexpr int ST = (W == 32) ? 2 : 1;                  // ring entries per evaluation step of one lane
     constexpr int BATCH_ITERS = FF_WALK_BATCH / ST;        // evaluation steps per batch of ring entries
@@ -189,6 +189,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
             if (QUAD) { sm.pendQ0[slot] = Q0; sm.pendQ1[slot] = Q1; }
         }
         pend_cnt += __popc(m);
+        FF_CHECK(g, pend_cnt <= FF_WALK_PEND);
     };
     auto drain = [&]() {
         while (pend_cnt >= FF_WALK_BATCH) {
@@ -241,6 +242,8 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
         }
         __syncwarp();
         const bool is_cell = e >= 0;
+        FF_CHECK(g, !is_cell || e < n_cells);
+        FF_CHECK(g, is_cell || e == FF_CHILD_EMPTY || (int)((uint32_t)e & FF_CHILD_SLOT) < n);
         const bool is_leaf = !is_cell && e != FF_CHILD_EMPTY;
         const bool is_multi = is_leaf && ((uint32_t)e & FF_CHILD_MULTI);
         const bool is_part = is_leaf && !is_multi;
@@ -309,6 +312,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
         }
         if (!full) {
             const unsigned pm = __ballot_sync(FF_FULL, park);
+            FF_CHECK(g, amb_cnt + __popc(pm) <= 64);
             if (park) sm.amb[amb_cnt + __popc(pm & lt)] = e;
             amb_cnt += __popc(pm);
         }
@@ -348,6 +352,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(FF_FULL, incl, o); if (lane >= o) incl += y; }
         const int total = __shfl_sync(FF_FULL, incl, 31);
+        FF_CHECK(g, sp_top + total <= FF_WALK_STACK && nch <= 8);
         {
             int32_t* w = sm.stack + (sp_top + incl - nch);
             if (nch > 0) w[0] = c0.x;
@@ -417,6 +422,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
     // walk makes ptxas rebuild the register pairs with MOVs inside the evaluation loop)
     auto store = [&](int k, float ux, float uy, float uz, float hx, float hy, float hz, float fvx, float fvy, float fvz,
                      float sk) {
+        FF_CHECK(g, k >= 0 && k < n && __ldg(perm + k) < (uint32_t)n);
         const size_t o = (size_t)__ldg(perm + k) * 3;      // a7: back to caller order;  f = fv + sk u_k
         if (H_out) { H_out[o] = hx; H_out[o + 1] = hy; H_out[o + 2] = hz; }
         if (F_out) { F_out[o] = fmaf(sk, ux, fvx); F_out[o + 1] = fmaf(sk, uy, fvy); F_out[o + 2] = fmaf(sk, uz, fvz); }
@@ -463,7 +469,7 @@ ff_k_walk(int n, int group_begin, int group_end, float theta, ff_globals* __rest
         grp = __shfl_sync(FF_FULL, grp, 0);
         if (grp >= groups) break;
         ff_walk_group<W, COUNT, BUCKET, QUAD>(sm, grp, lane, n, theta, n_cells, pos_s, mom_s, perm, cell_info, cell_child,
-                                              leaf_count, centre, moment, quad, H_out, F_out, counters);
+                                              leaf_count, centre, moment, quad, H_out, F_out, counters, g);
         __syncwarp();
     }
 }

@@ -3,6 +3,12 @@
     compute-sanitizer --tool memcheck  python tests/sanitizer_smoke.py
     compute-sanitizer --tool racecheck python tests/sanitizer_smoke.py
 
+or, where compute-sanitizer is not available, against the CHECKED build of the library (every kernel compiled with its
+device-side index and bound checks, FF_CHECK in csrc/ff_internal.cuh; a failed check makes the next ff_get_timings /
+ff_get_counters call return FF_ERR_CHECK with the source line):
+
+    FF_CHECKED=1 python tests/sanitizer_smoke.py
+
 Covers ff_build_tree, ff_eval_bh (N_leaf 1, 2 and 4, ragged N, counters on and off, W = 32 and 64, cell order 0 and 1),
 ff_eval_bh_range,
 ff_eval_direct (split and unsplit grids), ff_eval_bh_host and ff_step with Lennard-Jones pairs + walls, Barnes-Hut
@@ -56,10 +62,13 @@ def main():
             for s in range(2):
                 ctx.step(x, v, u, w, p, s)
         torch.cuda.synchronize()
+        ctx.timings()                                      # raises FFError if a device-side check failed (checked build)
         same = bool(torch.equal(H, H2) and torch.equal(F, F2))
         print("N=%d nleaf=%d W=%d order=%d: ranges compose=%s, BH vs direct rel L2 %.3e, finite=%s"
               % (N, nleaf, group, order, same, float((H - Hd).norm() / Hd.norm()), bool(torch.isfinite(x).all())))
         assert same
+    print("library: %s; no device-side error flag was raised" % ("CHECKED build (FF_CHECK compiled in)"
+                                                               if os.environ.get("FF_CHECKED") == "1" else "release build"))
 
 
 if __name__ == "__main__":

@@ -10,6 +10,8 @@ Tolerances (BASELINE.json north_star; error metric of DESIGN.md, reading Q19):
   those use the second metric only.
   keys, permutation, root cube, cell topology, cell centres/moments .......... bit exact
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -505,3 +507,17 @@ def test_config4_chains_sampled(ff):
 def test_config5_sixteen_million_sampled(ff):
     # N = 2^24, phi = 0.2, theta = 0.6: the HBM-resident case; the oracle walks 64 sampled groups
     _sampled_parity(ff, ffgen.config(5), 64)
+
+
+@pytest.mark.gpu
+def test_checked_build_raises_no_device_side_check():
+    """tests/sanitizer_smoke.py against libff_checked.so (-DFF_CHECKED: index and bound checks in every kernel); the
+    stand-in for a compute-sanitizer run where that tool is not available."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, FF_CHECKED="1")
+    out = subprocess.run([sys.executable, os.path.join(root, "tests", "sanitizer_smoke.py")], env=env, cwd=root,
+                         capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-2000:]
+    assert "CHECKED build" in out.stdout
