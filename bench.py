@@ -35,14 +35,15 @@ import numpy as np
 
 METRIC = "dipole field+force particle-evals/s (Barnes-Hut step: sort+build+moments+walk), N=2^20, theta=0.5"
 UNIT = "particle-evals/s"
-FLOP_PER_INTERACTION = 60.0      # 21 FFMA x2 + 17 FADD/FMUL + 1 MUFU.RSQ per h+f pair term
+FLOP_PER_INTERACTION = 60.0      # SURVEY.md 8(d)'s algorithmic figure per h+f pair term (the tensor form of ff_pair.cuh
+                                 # executes 25 FFMA x 2 + 11 FMUL = 61 per interaction, + 1 MUFU.RSQ)
 FP32_LANES_PER_SM = 128
 # algorithmic bytes per particle of the HBM-bound phases (DESIGN.md section 5 / SURVEY.md 8(d))
 ALG_BYTES = {"bbox_keys": 12 + 12 + 4, "sort": 4 * 16 + 4 + 12 + 16, "build": 26 + 16 * 0.39, "moments": 12 + 16 + 122}
 # dram__bytes_read.sum + dram__bytes_write.sum of one ff_k_walk launch at config 3, from the
 # `ncu --set full` capture summarised in profiles/r2_walk_full.md (a capture, not a measurement of this run)
-WALK_DRAM_TRAFFIC_BYTES = 107945472   # 86.60 MB read + 21.34 MB written
-WALK_DRAM_TRAFFIC_SOURCE = "ncu --set full capture of ff_k_walk<32,0,0> at commit 5a0c1f2, profiles/r2_walk_full.md"
+WALK_DRAM_TRAFFIC_BYTES = 108625920   # 86.91 MB read + 21.72 MB written
+WALK_DRAM_TRAFFIC_SOURCE = "ncu --set full capture of ff_k_walk<32,0,0,0> at commit 4ffcb26, profiles/r2_walk_full.md"
 
 
 def _peaks():
@@ -492,14 +493,14 @@ def run_ours(args):
         "interactions_per_launch": interactions, "flop_per_interaction": FLOP_PER_INTERACTION,
         "kernel_ms": walk_ms, "kernel_share_of_step": walk_ms / ms_per_step,
         "interactions_per_s": interactions / (walk_ms * 1e-3),
-        # FP32-pipe occupancy by the interaction arithmetic alone = interactions x 38 FP32 lane-ops
-        # (19 packed instructions of two lanes' worth each) / (time x SMs x 128 lanes x clock)
-        "fp32_lane_ops_per_interaction": 38,
-        "fp32_lane_occupancy_by_interactions": interactions * 38.0 / (walk_ms * 1e-3 * num_sms * FP32_LANES_PER_SM * sm_max * 1e6),
-        "note": "21 of the 38 FP32 instructions per interaction are FMAs, so a saturated FP32 pipe reads 0.78; the "
-                "register file feeds one even and one odd register per lane and cycle, so packed FMAs with three "
-                "register-pair operands issue every 3 cycles (ffma2_three_register_pairs), which caps this instruction "
-                "mix at eval_loop_ceiling_frac: the evaluation loop of the walk run alone",
+        # FP32-pipe occupancy by the interaction arithmetic alone = interactions x 36 FP32 lane-ops
+        # (18 packed instructions of two lanes' worth each) / (time x SMs x 128 lanes x clock)
+        "fp32_lane_ops_per_interaction": 36,
+        "fp32_lane_occupancy_by_interactions": interactions * 36.0 / (walk_ms * 1e-3 * num_sms * FP32_LANES_PER_SM * sm_max * 1e6),
+        "note": "25 of the 36 FP32 instructions per interaction are FMAs, so a saturated FP32 pipe reads 0.85; the "
+                "register file feeds a packed instruction two register words per lane and cycle, so packed FMAs with "
+                "three register-pair operands issue every 3 cycles (ffma2_three_register_pairs; 12 of the 36), which "
+                "caps this instruction mix at eval_loop_ceiling_frac: the evaluation loop of the walk run alone",
     }
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     # algorithmic bytes per particle of the HBM-bound phases (DESIGN.md / SURVEY.md 8(d))
