@@ -290,7 +290,7 @@ int ff_measure_fp32_peak(ff_ctx* ctx, int iters, double* tflops);
  *   FF_PROBE_FFMA2_PAIRS   packed FFMA2 with three distinct register-pair operands
  *   FF_PROBE_FFMA2_REUSE   packed FFMA2 with one operand shared by consecutive instructions (operand reuse cache)
  *   FF_PROBE_FFMA2_SCALAR  packed FFMA2 with one scalar operand in the broadcast form (how the sources enter Eq. 11-12)
- *   FF_PROBE_EVAL          the evaluation loop of the walk alone: 38 packed FP32 instructions + 2 MUFU.RSQ per source
+ *   FF_PROBE_EVAL          the evaluation loop of the walk alone: 36 packed FP32 instructions (force as a tensor) + 2 MUFU.RSQ per source
  *                          and pair of targets on shared-memory records, 60 flop per interaction -- the ceiling of the
  *                          walk and of the direct kernel
  */

@@ -91,10 +91,6 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
     const int tiles = (n + FF_BUILD_TILE - 1) / FF_BUILD_TILE;
     const int tpb = (tiles + gridDim.x - 1) / gridDim.x;
     const int t0 = min(tiles, (int)blockIdx.x * tpb), t1 = min(tiles, t0 + tpb);
-#ifdef FF_BUILD_PROFILE
-    unsigned long long tq[4];
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tq[0]));
-#endif
 
     // ---- phase 1
     {
@@ -119,9 +115,6 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
     // by now): saves a reset launch per step; ff_create and a failed call run ff_k_reset instead
     if (blockIdx.x == gridDim.x - 1) ff_reset_globals(g, threadIdx.x, FF_BUILD_THREADS);
     grid.sync();
-#ifdef FF_BUILD_PROFILE
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tq[1]));
-#endif
 
     // ---- phase 2
     {
@@ -185,9 +178,6 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
         if (threadIdx.x < FF_MAX_LEVEL && s_hist[threadIdx.x]) atomicAdd(&g->level_count[threadIdx.x], s_hist[threadIdx.x]);
     }
     grid.sync();
-#ifdef FF_BUILD_PROFILE
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tq[2]));
-#endif
 
     // ---- phase 3
     // Latency bound (three dependent loads per cell: first slot -> window keys -> cell_base of the children), so every
@@ -303,12 +293,6 @@ ff_k_build(const uint32_t* __restrict__ key, int n, int nleaf, uint32_t* __restr
             }
         }
     }
-#ifdef FF_BUILD_PROFILE
-    grid.sync();
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tq[3]));
-    if (blockIdx.x == 0 && threadIdx.x == 0)
-        printf("build phases ns: p1 %llu p2 %llu p3 %llu (n_cells %d)\n", tq[1] - tq[0], tq[2] - tq[1], tq[3] - tq[2], g->n_cells);
-#endif
 }
 
 // ---- a5: Eq. 14: ONE cooperative launch -----------------------

@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(256) ff_k_keys(const float* __restrict__ pos, 
 // count at once and its inclusive prefix as soon as it knows it).  Tiles are handed out by an
 // atomic ticket, so every tile a block waits for is already running.  Stable: a warp owns a
 // contiguous chunk and walks it in rounds of 32; rank = earlier tiles + earlier warps + earlier
-// rounds + lower lanes (warp match).
+// rounds + lower lanes with the same digit (peer mask from a shared-memory word per warp and digit).
 #ifndef FF_SORT_WINDOW
 #define FF_SORT_WINDOW 8
 #endif
@@ -157,23 +157,31 @@ ff_k_radix_onesweep(const uint32_t* __restrict__ kin, const uint32_t* __restrict
         key[r] = valid ? __ldg(kin + i) : 0xffffffffu;
         val[r] = valid ? (vin ? __ldg(vin + i) : (uint32_t)i) : 0u;
     }
+    // Stable ranking inside the warp's chunk.  The lanes of a round that hold the same digit find each other through a
+    // shared-memory word per (warp, digit): every lane ORs its lane bit in, reads the word back (= the peer mask), the
+    // lowest peer bumps the warp's running count of that digit and clears the word for the next round.  One
+    // shared-memory atomic per key instead of eight ballots with their mask arithmetic (the sort passes are
+    // instruction bound, profiles/r2_hbm_phases.md).  The words live in `skey`, which is not needed before the
+    // ranking is done.
+    uint32_t* match = skey + w * FF_RADIX;
+    static_assert(FF_SORT_TILE >= (FF_SORT_THREADS / 32) * FF_RADIX, "the match words of all warps fit in skey");
+#pragma unroll
+    for (int k = 0; k < FF_RADIX / 32; ++k) match[k * 32 + lane] = 0u;
+    __syncwarp();
 #pragma unroll
     for (int r = 0; r < FF_SORT_ROUNDS; ++r) {
-        bool valid = base + r * 32 + lane < n;
-        uint32_t d = (key[r] >> shift) & (FF_RADIX - 1);
-        // lanes with the same digit, from eight ballots (much faster than MATCH.ANY with ~28 distinct digits per warp)
-        unsigned peers = __ballot_sync(FF_FULL, valid);
-#pragma unroll
-        for (int b = 0; b < FF_RADIX_BITS; ++b) {
-            unsigned bal = __ballot_sync(FF_FULL, (d >> b) & 1u);
-            peers &= ((d >> b) & 1u) ? bal : ~bal;
-        }
-        int leader = __ffs(peers) - 1;
-        uint32_t old = 0;
-        if (valid && lane == leader) { old = wh[w][d]; wh[w][d] = old + (uint32_t)__popc(peers); }
-        old = __shfl_sync(FF_FULL, old, leader);
-        rank[r] = old + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+        const bool valid = base + r * 32 + lane < n;
+        const uint32_t d = (key[r] >> shift) & (FF_RADIX - 1);
+        if (valid) atomicOr(&match[d], 1u << lane);
         __syncwarp();
+        const unsigned peers = valid ? match[d] : 0u;
+        const int leader = __ffs(peers) - 1;
+        uint32_t old = 0;
+        __syncwarp();                                      // every peer has read the word before its leader clears it
+        if (valid && lane == leader) { old = wh[w][d]; wh[w][d] = old + (uint32_t)__popc(peers); match[d] = 0u; }
+        old = __shfl_sync(FF_FULL, old, leader < 0 ? 0 : leader);
+        rank[r] = old + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+        __syncwarp();                                      // the cleared word before the next round's ORs
     }
     __syncthreads();
     // digit t: count of this tile; per-warp counts become offsets inside the tile's run of digit t
