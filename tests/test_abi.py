@@ -38,6 +38,7 @@ def test_host_side_argument_checks_without_gpu():
     assert L.ff_destroy(None) == ff.FF_ERR_INVALID_ARG
     assert L.ff_build_tree(None, None, 1) == ff.FF_ERR_INVALID_ARG
     assert L.ff_error_string(ff.FF_ERR_NO_TREE).decode().startswith("no tree")
+    assert "check" in L.ff_error_string(ff.FF_ERR_CHECK).decode()
     assert ctypes.sizeof(ff.ff_step_params) == 96 and ctypes.sizeof(ff.ff_tree_view) == 136
 
 
@@ -53,3 +54,11 @@ def test_product_never_imports_the_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_1212_2934_b200 import" not in src and "import paper_1212_2934_b200" not in src
             assert "csrc" not in src.replace("paper_1212_2934_b200/csrc (the CUDA path)", "")
+
+
+def test_checked_library_builds_and_exports_the_same_symbols():
+    """libff_checked.so (-DFF_CHECKED: device-side index and bound checks in every kernel) is the same ABI."""
+    from paper_1212_2934_b200 import build
+    L = ctypes.CDLL(build.build(checked=True))
+    for n in _declared():
+        assert hasattr(L, n), n
