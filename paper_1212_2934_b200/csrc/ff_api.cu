@@ -72,8 +72,11 @@ static void ff_teardown(ff_ctx* c)
         if (c->ev_done[b]) cudaEventDestroy(c->ev_done[b]);
         if (c->ev_out[b]) cudaEventDestroy(c->ev_out[b]);
     }
+    if (c->ev_tree) cudaEventDestroy(c->ev_tree);
+    if (c->ev_lj) cudaEventDestroy(c->ev_lj);
     if (c->in_stream) cudaStreamDestroy(c->in_stream);
     if (c->out_stream) cudaStreamDestroy(c->out_stream);
+    if (c->lj_stream) cudaStreamDestroy(c->lj_stream);
     delete c;
 }
 
@@ -96,6 +99,13 @@ extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, 
         for (int k = 0; e == cudaSuccess && k < 2; ++k) e = cudaEventCreate(&c->ev[ph][k]);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->in_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->out_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) {
+        int least = 0, greatest = 0;                       // the lowest priority: the walk's blocks go first
+        e = cudaDeviceGetStreamPriorityRange(&least, &greatest);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&c->lj_stream, cudaStreamNonBlocking, least);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_tree, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_lj, cudaEventDisableTiming);
     for (int b = 0; e == cudaSuccess && b < 2; ++b) {
         e = cudaEventCreateWithFlags(&c->ev_pos[b], cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_in[b], cudaEventDisableTiming);
@@ -115,6 +125,7 @@ extern "C" int ff_destroy(ff_ctx* c)
     cudaStreamSynchronize(c->stream);
     if (c->in_stream) cudaStreamSynchronize(c->in_stream);
     if (c->out_stream) cudaStreamSynchronize(c->out_stream);
+    if (c->lj_stream) cudaStreamSynchronize(c->lj_stream);
     ff_teardown(c);
     return FF_OK;
 }
@@ -300,18 +311,28 @@ extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* ang
         if ((rc = ff_launch_direct(c, pos, mom, n, c->stage_H, c->stage_F, p->lj_epsilon, p->lj_sigma, p->lj_cutoff)) != FF_OK)
             return rc;
         ff_phase_end(c, FF_PH_DIRECT);
-        ff_step_params q = *p;
-        q.lj_epsilon = 0.0f;                                       // already inside stage_F
-        ff_phase_begin(c, FF_PH_STEP);
-        if ((rc = ff_launch_step(c, pos, vel, mom, angvel, n, &q, step_index)) != FF_OK) return rc;
+        ff_phase_begin(c, FF_PH_STEP);                             // (f^sr is already inside stage_F)
+        if ((rc = ff_launch_integrate(c, pos, vel, mom, angvel, n, p, step_index, false)) != FF_OK) return rc;
         ff_phase_end(c, FF_PH_STEP);
         c->tree_built = 0;
         return FF_OK;
     }
+    // The Lennard-Jones pass needs the tree (sorted keys and positions), not the fields: it is enqueued on its own
+    // low-priority stream AFTER the walk and runs beside it, in the SMs the persistent walk leaves idle while it drains
+    // (about 0.17 ms at N = 2^20, profiles/r2_walk_full.md); the update waits for both.
+    const bool lj = p->lj_epsilon != 0.0f;
+    if (lj && (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
     if ((rc = ff_build_tree(c, pos, n)) != FF_OK) return rc;
+    if (lj) FF_CUDA(c, cudaEventRecord(c->ev_tree, c->stream));
     if ((rc = ff_eval_bh(c, pos, mom, c->stage_H, c->stage_F)) != FF_OK) return rc;
     ff_phase_begin(c, FF_PH_STEP);
-    if ((rc = ff_launch_step(c, pos, vel, mom, angvel, n, p, step_index)) != FF_OK) return rc;
+    if (lj) {
+        FF_CUDA(c, cudaStreamWaitEvent(c->lj_stream, c->ev_tree, 0));
+        if ((rc = ff_launch_lj(c, n, p, c->lj_stream)) != FF_OK) return rc;
+        FF_CUDA(c, cudaEventRecord(c->ev_lj, c->lj_stream));
+        FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_lj, 0));
+    }
+    if ((rc = ff_launch_integrate(c, pos, vel, mom, angvel, n, p, step_index, lj)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_STEP);
     c->tree_built = 0;                // positions moved: the tree no longer matches
     return FF_OK;

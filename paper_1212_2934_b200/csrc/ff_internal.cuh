@@ -91,6 +91,10 @@ struct ff_ctx {
     // buffers and events double-buffered by call parity (ff_api.cu)
     cudaStream_t in_stream, out_stream;
     cudaEvent_t ev_pos[2], ev_in[2], ev_done[2], ev_out[2];
+    // ff_step: the Lennard-Jones pass needs the tree only, not the walk's results; it runs on its own low-priority
+    // stream beside the walk and fills the SMs the draining walk leaves idle (ff_api.cu)
+    cudaStream_t lj_stream;
+    cudaEvent_t ev_tree, ev_lj;
     uint64_t host_seq;                // *_host calls issued so far
     uint64_t launches;
     char last_error[256];
@@ -174,8 +178,9 @@ int ff_launch_walk(ff_ctx* c, float* H_out, float* F_out, int group_begin = 0, i
 int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n, float* H_out, float* F_out,
                      float lj_eps = 0.0f, float lj_sigma = 1.0f, float lj_cutoff = 0.0f);   // lj_eps != 0: F_out = f^dip + f^sr
 int ff_launch_probe(ff_ctx* c, int kind, int iters, double* tflops);
-int ff_launch_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n,
-                   const ff_step_params* p, uint64_t step_index);
+int ff_launch_lj(ff_ctx* c, int64_t n, const ff_step_params* p, cudaStream_t stream);   // -> c->step_fsr (needs the tree)
+int ff_launch_integrate(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n,
+                        const ff_step_params* p, uint64_t step_index, bool with_fsr);
 
 // ---- checked build (-DFF_CHECKED): device-side index and bound checks of every kernel --------------------------
 // compute-sanitizer is not available on every machine this runs on; the checked library is what

@@ -176,24 +176,36 @@ ff_k_integrate(int n, float* __restrict__ pos, float* __restrict__ vel, float* _
     for (int a = 0; a < 3; ++a) mom[o + a] = un[a] * inv;
 }
 
-int ff_launch_step(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n64,
-                   const ff_step_params* p, uint64_t step_index)
+// Eq. 13 over the pairs within the cut-off -> c->step_fsr, enqueued on `stream`.  Reads the sorted keys and positions
+// of the current tree only.
+int ff_launch_lj(ff_ctx* c, int64_t n64, const ff_step_params* p, cudaStream_t stream)
 {
-    int n = (int)n64;
-    const float* fsr = nullptr;
-    if (p->wall_epsilon != 0.0f && (!(p->lj_cutoff > 0.0f) || !(p->wall_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
-    if (p->lj_epsilon != 0.0f) {
-        if (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f)) return FF_ERR_INVALID_ARG;
-        size_t cells = (size_t)1 << (3 * FF_LJ_MAX_LEVEL);                   // table sized for the deepest level
-        int32_t* start = reinterpret_cast<int32_t*>(c->direct_part);       // 2 * 8^7 * 4 B = 16 MB <= scratch
-        int32_t* end = start + cells;
+    const int n = (int)n64;
+    if (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f)) return FF_ERR_INVALID_ARG;
+    const size_t cells = (size_t)1 << (3 * FF_LJ_MAX_LEVEL);                // table sized for the deepest level
+    int32_t* start = reinterpret_cast<int32_t*>(c->direct_part);          // 2 * 8^7 * 4 B = 16 MB <= scratch
+    int32_t* end = start + cells;
+    const cudaStream_t main_stream = c->stream;
+    c->stream = stream;                                                    // FF_LAUNCH enqueues on c->stream
+    int rc = FF_OK;
+    auto enqueue = [&]() -> int {
         FF_CUDA(c, cudaMemsetAsync(start, 0, 2 * cells * sizeof(int32_t), c->stream));
         FF_LAUNCH(c, ff_k_cell_table, (n + 255) / 256, 256, 0, c->key[0], n, c->g, p->lj_cutoff, start, end);
         FF_LAUNCH(c, ff_k_lj, (n + 127) / 128, 128, 0, c->key[0], c->pos_s, c->idx[0], n, c->g, start, end,
                   p->lj_epsilon, p->lj_sigma, p->lj_cutoff, c->step_fsr);
-        fsr = c->step_fsr;
-    }
-    FF_LAUNCH(c, ff_k_integrate, (n + 255) / 256, 256, 0, n, pos, vel, mom, angvel, c->stage_H, c->stage_F, fsr, *p,
-              step_index);
+        return FF_OK;
+    };
+    rc = enqueue();
+    c->stream = main_stream;
+    return rc;
+}
+
+int ff_launch_integrate(ff_ctx* c, float* pos, float* vel, float* mom, float* angvel, int64_t n64,
+                        const ff_step_params* p, uint64_t step_index, bool with_fsr)
+{
+    const int n = (int)n64;
+    if (p->wall_epsilon != 0.0f && (!(p->lj_cutoff > 0.0f) || !(p->wall_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
+    FF_LAUNCH(c, ff_k_integrate, (n + 255) / 256, 256, 0, n, pos, vel, mom, angvel, c->stage_H, c->stage_F,
+              with_fsr ? c->step_fsr : (const float*)nullptr, *p, step_index);
     return FF_OK;
 }
