@@ -521,3 +521,15 @@ def test_checked_build_raises_no_device_side_check():
                          capture_output=True, text=True, timeout=900)
     assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-2000:]
     assert "CHECKED build" in out.stdout
+
+
+@pytest.mark.gpu
+def test_checked_build_catches_a_corrupted_tree():
+    """Negative control: the device-side checks of libff_checked.so do fire (tests/checked_negative_control.py)."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "tests", "checked_negative_control.py")],
+                         env=dict(os.environ, FF_CHECKED="1"), cwd=root, capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-2000:]
+    assert "caught the corrupted permutation" in out.stdout
