@@ -188,6 +188,9 @@ int ff_eval_direct_host(ff_ctx* ctx, const float* pos_host, const float* mom_hos
  * All arrays device [n][3] fp32.  noise_* = 0 gives the deterministic step
  * used by the parity tests; otherwise xi are unit Gaussians from a
  * counter-based generator keyed by (seed, step_index, particle, component).
+ * Streams: the call is ordered on the context's stream like every other call (work enqueued on that stream after
+ * ff_step returns sees the updated state).  Internally the Lennard-Jones pass, which needs the tree but not the
+ * fields, runs on a second, low-priority stream of the context beside the tree walk; the update waits for both.
  */
 typedef struct ff_step_params {
     float dtau;          /* time step (paper: 0.001) */
