@@ -123,6 +123,26 @@ def test_ragged_sizes(ff, N):
         assert np.all(Hd.cpu().numpy() == 0) and np.all(Fd.cpu().numpy() == 0)
 
 
+@pytest.mark.parametrize("scale,shift", [(1e-3, 0.0), (1e3, 0.0), (1e5, -3e7), (1.0, 1e4)])
+def test_length_scale_and_offset(ff, scale, shift):
+    """The path is unit free (H ~ L^-3, F ~ L^-4, SURVEY.md 8(b) "Units"): the same ensemble in another length unit
+    and far from the origin, with moments that are not unit vectors (Eq. 11-12 are bilinear in them).  The oracle is
+    evaluated on the very same fp32 inputs, so this checks the fp32 range and the cancellation in rho = p_k - p_j, not a
+    scaling law."""
+    c = ffgen.config(1, N=3000, seed=5)
+    pos = (c["pos"].astype(np.float64) * scale + shift).astype(np.float32)
+    mom = (c["mom"] * np.float32(2.5)).astype(np.float32)
+    ctx, H, F = _gpu_bh(ff, pos, mom, 0.5)
+    Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, 0.5, 32, scale=True)
+    _check_tree(ff, ctx, otree, otree.moments(mom))
+    assert ctx.counters() == cnt
+    assert np.isfinite(H).all() and np.isfinite(F).all()
+    check_hf(H, F, Ho, Fo, Q, TOL_BH)
+    Hd, Fd = ctx.eval_direct(_dev(pos), _dev(mom))
+    Ha, Fa, Qa = oracle.allpairs(pos, mom, scale=True)
+    check_hf(Hd.cpu().numpy(), Fd.cpu().numpy(), Ha, Fa, Qa, TOL_DIRECT)
+
+
 @pytest.mark.parametrize("nleaf", [1, 2, 8, 32, 100])
 def test_leaf_capacity(ff, nleaf):
     c = ffgen.config(1, N=1500, seed=3)
