@@ -52,9 +52,10 @@ typedef enum ff_status {
     FF_ERR_CAPACITY = -4,       /* internal pool overflow (cannot happen with ff_workspace_bytes' sizing; kept for the ABI).
                                    Detected on the device, reported by the next ff_get_tree / ff_get_timings / ff_get_counters */
     FF_ERR_CUDA = -5,           /* CUDA runtime / launch failure; text via ff_last_error */
-    FF_ERR_CHECK = -6           /* checked build only (library compiled with -DFF_CHECKED): a device-side index or bound
+    FF_ERR_CHECK = -6,          /* checked build only (library compiled with -DFF_CHECKED): a device-side index or bound
                                    check failed; reported like FF_ERR_CAPACITY, the failing source line is in
                                    ff_last_error after the reporting call */
+    FF_ERR_TOO_LARGE = -7       /* ff_eval_direct_static only: n > FF_STATIC_MAX_N (its scratch array has a fixed size) */
 } ff_status;
 
 #define FF_MAX_N (1ll << 28)    /* particle slots must fit the 30-bit stack entries of the walk */
@@ -152,6 +153,39 @@ int ff_eval_bh_range(ff_ctx* ctx, const float* pos, const float* mom, float* H_o
  * index (line 5).  Needs no tree.  Arguments as ff_eval_bh, n given.
  */
 int ff_eval_direct(ff_ctx* ctx, const float* pos, const float* mom, int64_t n, float* H_out, float* F_out);
+
+/*
+ * The same all-pairs sum (a8, Algorithm 1) for callers that must not allocate device memory.
+ *
+ * Who that is: code that runs after a framework's memory pool has claimed the whole GPU, so that a cudaMalloc of
+ * its own fails or fights the pool; code inside a latency-critical loop, where cudaMalloc / cudaFree stall the
+ * whole device; and plug-ins that are handed fixed input and output buffers and nothing they could use as the
+ * workspace ff_create asks for.  For n of a few thousand the all-pairs kernel splits the sources over the grid and
+ * needs somewhere to keep one fp64 partial sum per (split, target) until they are added up; ff_eval_direct keeps
+ * them in the caller's workspace, this call keeps them in an array that is compiled into the library.
+ *
+ *  - No context, no workspace; the call makes no cudaMalloc, cudaFree or other allocating call.  The array is
+ *    3 MiB of device memory that EVERY GPU on which this library gets loaded holds until the process exits,
+ *    whether or not this function is ever called there.
+ *  - n <= FF_STATIC_MAX_N (what the array can hold); a larger n returns FF_ERR_TOO_LARGE and launches nothing.
+ *  - pos, mom: device [n][3] fp32; H_out, F_out: device [n][3] fp32, one of them may be NULL.  All arrays and
+ *    cuda_stream (a cudaStream_t; NULL = default stream) must belong to the CURRENT device; the work is
+ *    enqueued on that stream and the call returns without synchronising.
+ *  - The first call on each device looks up the array's device address (cudaGetSymbolAddress, which may also load
+ *    the library's kernels onto that device).  Make that first call outside any stream capture.
+ *  - All calls share the one array, and it keeps whatever the last call left in it.  That is harmless for calls
+ *    that follow one another on the GPU (every record a call reads it has written itself first; nothing relies on
+ *    zeros), but two calls whose kernels can run at the same time on one GPU -- different streams, no event
+ *    between them -- overwrite each other's partial sums and return garbage.  Order them yourself.
+ *  - Results: the same arithmetic as ff_eval_direct (the same kernels); they agree to rounding order, and bit for
+ *    bit whenever both pick the same number of source splits.
+ * Returns FF_OK or a negative ff_status; ff_static_last_error() has the text of this thread's last failure.
+ */
+#define FF_STATIC_MAX_N 32768
+int ff_eval_direct_static(const float* pos, const float* mom, int64_t n, float* H_out, float* F_out,
+                          void* cuda_stream);
+/* Text of the calling thread's last ff_eval_direct_static failure ("" after a success). */
+const char* ff_static_last_error(void);
 
 /*
  * End-to-end convenience calls with HOST buffers: copy pos/mom to the device

@@ -22,6 +22,8 @@ _lib = None
 
 FF_OK = 0
 FF_ERR_INVALID_ARG, FF_ERR_WORKSPACE, FF_ERR_NO_TREE, FF_ERR_CAPACITY, FF_ERR_CUDA, FF_ERR_CHECK = -1, -2, -3, -4, -5, -6
+FF_ERR_TOO_LARGE = -7
+FF_STATIC_MAX_N = 32768
 FF_OPT_THETA, FF_OPT_NLEAF, FF_OPT_COUNTERS, FF_OPT_TIMING, FF_OPT_GROUP, FF_OPT_CELL_ORDER = 1, 2, 3, 4, 5, 6
 FF_N_PHASES = 7
 PHASES = ("bbox_keys", "sort", "build", "moments", "walk", "direct", "step")
@@ -34,7 +36,7 @@ SYMBOLS = (
     "ff_workspace_bytes", "ff_create", "ff_destroy", "ff_set_stream", "ff_set_option", "ff_build_tree",
     "ff_eval_bh", "ff_eval_bh_range", "ff_eval_direct", "ff_eval_bh_host", "ff_eval_direct_host", "ff_step", "ff_get_tree",
     "ff_get_timings", "ff_eval_bh_host_async", "ff_host_sync", "ff_get_counters", "ff_get_prefilter_count", "ff_get_launch_count", "ff_measure_fp32_peak", "ff_measure_probe", "ff_error_string",
-    "ff_last_error",
+    "ff_last_error", "ff_eval_direct_static", "ff_static_last_error",
 )
 
 
@@ -127,6 +129,10 @@ def lib():
         L.ff_error_string.argtypes = [i32]
         L.ff_last_error.restype = ctypes.c_char_p
         L.ff_last_error.argtypes = [vp]
+        L.ff_eval_direct_static.restype = i32
+        L.ff_eval_direct_static.argtypes = [vp, vp, i64, vp, vp, vp]
+        L.ff_static_last_error.restype = ctypes.c_char_p
+        L.ff_static_last_error.argtypes = []
         _lib = L
     return _lib
 
@@ -143,6 +149,30 @@ def _dev_f32(t, n=None, name="tensor"):
     if n is not None and t.shape[0] != n:
         raise ValueError("%s has %d rows, expected %d" % (name, t.shape[0], n))
     return t.data_ptr()
+
+
+def eval_direct_static(pos, mom, H, F, stream=None):
+    """ff_eval_direct_static: exact all-pairs field and force for n <= FF_STATIC_MAX_N particles without a context,
+    a workspace or any device allocation -- the partial sums live in an array built into libff.so.  Meant for code
+    that may not call cudaMalloc where it runs (a memory pool owns the whole GPU, a latency-critical loop, a plug-in
+    that only gets fixed buffers).  The caller passes the outputs too (H or F may be None to skip one); nothing is
+    allocated here either.  `stream`: a raw cudaStream_t, default torch's current stream of pos.device.  Calls that
+    can overlap on the GPU share the array and race; see include/ff.h."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1212_2934_b200 needs a CUDA device: there is no CPU fallback")
+    n = pos.shape[0]
+    p, m = _dev_f32(pos, n, "pos"), _dev_f32(mom, n, "mom")
+    hp = _dev_f32(H, n, "H") if H is not None else None
+    fp = _dev_f32(F, n, "F") if F is not None else None
+    L = lib()
+    with torch.cuda.device(pos.device):
+        if stream is None:
+            stream = torch.cuda.current_stream(pos.device).cuda_stream
+        rc = L.ff_eval_direct_static(p, m, n, hp, fp, ctypes.c_void_p(stream))
+    if rc != FF_OK:
+        raise FFError(rc, "ff_eval_direct_static", L.ff_static_last_error().decode())
+    return H, F
 
 
 class FFContext:

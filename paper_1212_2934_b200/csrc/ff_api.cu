@@ -438,6 +438,7 @@ extern "C" const char* ff_error_string(int code)
     case FF_ERR_CAPACITY: return "cell pool capacity exceeded";
     case FF_ERR_CUDA: return "CUDA error (see ff_last_error)";
     case FF_ERR_CHECK: return "device-side check failed (checked build; see ff_last_error)";
+    case FF_ERR_TOO_LARGE: return "n is beyond FF_STATIC_MAX_N, the fixed limit of ff_eval_direct_static (see ff_static_last_error)";
     default: return "unknown error code";
     }
 }

@@ -181,3 +181,91 @@ int ff_launch_direct(ff_ctx* c, const float* pos, const float* mom, int64_t n64,
         FF_LAUNCH(c, ff_k_direct_reduce, (n + 255) / 256, 256, 0, c->direct_part, n, splits, H_out, F_out);
     return FF_OK;
 }
+
+// ---- ff_eval_direct_static: the all-pairs sum for callers that cannot allocate (include/ff.h) --------------------
+// The split kernel above parks one fp64 partial sum per (source split, target) in scratch before ff_k_direct_reduce
+// folds them.  Every other entry point takes that scratch from the caller's workspace; this one takes it from a
+// fixed array that is part of the library image, so it needs no context, no workspace and no allocation call.
+// The price: every GPU that loads libff.so carries these 3 MiB until the process exits, n is capped at
+// FF_STATIC_MAX_N, and all calls share the one array.
+#include <mutex>
+
+#define FF_STATIC_PART_ELEMS (2 * FF_STATIC_MAX_N)      // (split, target) pairs the array holds: 65 536 x 48 B = 3 MiB
+#define FF_STATIC_MAX_DEVICES 64
+
+static __device__ __align__(256) double ff_static_part[(size_t)FF_STATIC_PART_ELEMS * 6];
+
+namespace {
+// In host code `ff_static_part` is only a handle for the runtime, not an address a kernel can use: the device
+// address is asked for once per device (with that device current) and kept here.
+struct ff_static_dev { double* part; int num_sms; bool ready; };
+ff_static_dev ff_static_devs[FF_STATIC_MAX_DEVICES];
+std::mutex ff_static_mutex;
+thread_local char ff_static_error[256] = "";
+
+int ff_static_fail(int code, const char* what, const char* detail)
+{
+    snprintf(ff_static_error, sizeof(ff_static_error), "%s: %s", what, detail);
+    return code;
+}
+}   // namespace
+
+extern "C" const char* ff_static_last_error(void) { return ff_static_error; }
+
+extern "C" int ff_eval_direct_static(const float* pos, const float* mom, int64_t n, float* H_out, float* F_out,
+                                     void* cuda_stream)
+{
+    ff_static_error[0] = 0;
+    if (!pos || !mom || n <= 0 || (!H_out && !F_out))
+        return ff_static_fail(FF_ERR_INVALID_ARG, "ff_eval_direct_static", "NULL pos/mom, n <= 0 or no output array");
+    if (n > FF_STATIC_MAX_N) {
+        char msg[160];
+        snprintf(msg, sizeof(msg), "n = %lld is beyond FF_STATIC_MAX_N = %d, the most the built-in scratch array holds; "
+                 "use ff_eval_direct with a workspace", (long long)n, (int)FF_STATIC_MAX_N);
+        return ff_static_fail(FF_ERR_TOO_LARGE, "ff_eval_direct_static", msg);
+    }
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return ff_static_fail(FF_ERR_CUDA, "cudaGetDevice", cudaGetErrorString(e));
+    if (dev < 0 || dev >= FF_STATIC_MAX_DEVICES)
+        return ff_static_fail(FF_ERR_INVALID_ARG, "ff_eval_direct_static", "device ordinal beyond FF_STATIC_MAX_DEVICES");
+    ff_static_dev sd;
+    {
+        // first call on this device: look the array's device address up (this may load the module's kernels, which
+        // is why the first call belongs before any stream capture)
+        std::lock_guard<std::mutex> lock(ff_static_mutex);
+        ff_static_dev& slot = ff_static_devs[dev];
+        if (!slot.ready) {
+            double* p = nullptr;
+            e = cudaGetSymbolAddress((void**)&p, ff_static_part);
+            if (e != cudaSuccess || !p)
+                return ff_static_fail(FF_ERR_CUDA, "cudaGetSymbolAddress(ff_static_part)", cudaGetErrorString(e));
+            int sms = 0;
+            e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e != cudaSuccess || sms <= 0)
+                return ff_static_fail(FF_ERR_CUDA, "cudaDeviceGetAttribute(multiProcessorCount)", cudaGetErrorString(e));
+            slot.part = p; slot.num_sms = sms; slot.ready = true;
+        }
+        sd = slot;
+    }
+    // the grid of ff_launch_direct, with the split count bounded by what the array holds.  Nothing in the array has
+    // to start at zero: block (bx, by) overwrites all six sums of each of its (by, k) records, and the reduction
+    // reads only records [0, splits) x [0, n), so what an earlier call left behind is never read.
+    const int ni = (int)n;
+    const int tblocks = (ni + FF_DIRECT_TARGETS - 1) / FF_DIRECT_TARGETS;
+    const int n_tiles = (ni + FF_DIRECT_THREADS - 1) / FF_DIRECT_THREADS;
+    int splits = (sd.num_sms * 4 + tblocks - 1) / tblocks;
+    if (splits > n_tiles) splits = n_tiles;
+    if ((int64_t)splits * ni > FF_STATIC_PART_ELEMS) splits = (int)(FF_STATIC_PART_ELEMS / ni);
+    if (splits < 1) splits = 1;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    const ff_lj lj = { 0.0f, 1.0f, 0.0f };
+    ff_k_direct<false><<<dim3(tblocks, splits), FF_DIRECT_THREADS, 0, stream>>>(pos, mom, ni, splits, sd.part, H_out, F_out, lj);
+    if ((e = cudaGetLastError()) != cudaSuccess) return ff_static_fail(FF_ERR_CUDA, "ff_k_direct", cudaGetErrorString(e));
+    if (splits > 1) {
+        ff_k_direct_reduce<<<(ni + 255) / 256, 256, 0, stream>>>(sd.part, ni, splits, H_out, F_out);
+        if ((e = cudaGetLastError()) != cudaSuccess)
+            return ff_static_fail(FF_ERR_CUDA, "ff_k_direct_reduce", cudaGetErrorString(e));
+    }
+    return FF_OK;
+}
