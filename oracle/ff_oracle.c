@@ -22,6 +22,11 @@
  *   ffo_bh_eval ......... theta = 0 == all-pairs, N <= N_leaf == all-pairs,
  *                         independently written recursive list builder on
  *                         N <= 64, far-cluster limit, (28 pi/3) theta^-3 count
+ *   member_accepts ...... the opening test ON its threshold (tests/test_oracle_walk.py): exact equality
+ *                         s^2 == theta^2 d2 opens, one fp32 step beyond accepts, one short opens, and two
+ *                         targets found by a seeded search on which the fused order of O5 and three rounded
+ *                         squares added left to right decide differently (decisions taken from exact-rational
+ *                         fma in tests/helpers.py)
  *   Q output (scale) .... independent numpy sum of squared terms (all-pairs and the list builder's lists),
  *                         exact-rational closed form on the straight chain (tests/test_oracle_scale.py)
  *   first-order cell term (O1b, not in the paper): central differences of Eq. 11-12 in the source

@@ -280,3 +280,60 @@ def check_hf(H, F, Ho, Fo, Q, tol, survey=True):
         sh, sf = rel_err(H, Ho), rel_err(F, Fo)
         assert sh[0] <= tol and sf[0] <= tol, ("survey metric (no Q)", sh, sf)
     return eh, ef
+
+
+# ---- crafted inputs that sit ON the opening test's threshold (reading O5 / Q1) ----------------------------
+def opening_case(t, seed=0):
+    """35 particles around ONE decision: does group 0 (W = 32) accept the level-2 cell of the pair a, b?
+
+    Root cube [0, 8]^3 (a target at the origin, a particle at (8, 8, 8)), so s_2 = 2 and fl(s_2^2) = 4.  The pair
+    a = (4.5, 0.5, 1), b = (5.5, 1.5, 1) is alone in the level-2 cell [4,6) x [0,2) x [0,2); its centre (Eq. 14) is
+    exactly (5, 1, 1) in fp64 and in fp32.  Group 0 = the 32 particles of octant 0: 30 fillers in [0.05, 0.9]^3 and
+    the origin, all at d^2 >= 16.8 from the centre (they accept at theta = 0.5, where the rule reads 4 < d2 / 4),
+    and the critical target t, which alone decides.  Returns (pos, mom, slot_a, slot_b): caller-order fp32 arrays
+    and the caller indices of a and b."""
+    rng = np.random.default_rng(seed)
+    fill = rng.uniform(0.05, 0.9, (30, 3)).astype(np.float32)
+    pos = np.concatenate([fill, np.zeros((1, 3), np.float32), np.asarray(t, np.float32).reshape(1, 3),
+                          np.array([[4.5, 0.5, 1.0], [5.5, 1.5, 1.0], [8.0, 8.0, 8.0]], np.float32)])
+    u = rng.normal(size=(len(pos), 3))
+    mom = (u / np.linalg.norm(u, axis=1, keepdims=True)).astype(np.float32)
+    return pos, mom, 32, 33
+
+
+OPENING_CENTRE = np.array([5.0, 1.0, 1.0], np.float32)
+
+
+def opening_d2(t, fused=True):
+    """d2 of target t against OPENING_CENTRE in fp32: the order of reading O5 (fused: fma(dz,dz, fma(dy,dy, fl(dx dx))))
+    or the plausible mistake (three rounded squares added left to right)."""
+    f = np.float32
+    dx, dy, dz = (f(t[0]) - OPENING_CENTRE[0], f(t[1]) - OPENING_CENTRE[1], f(t[2]) - OPENING_CENTRE[2])
+    xx = f(dx * dx)
+    if fused:
+        return fmaf_exact(dz, dz, fmaf_exact(dy, dy, xx))
+    return f(f(xx + f(dy * dy)) + f(dz * dz))
+
+
+def fma_sensitive_targets(seed=1212, tries=4000):
+    """Seeded search for two critical targets on which the fused and the unfused d2 fall on different sides of the
+    threshold d2 > 16 (theta = 0.5, s_2 = 2): one the fused order accepts and the unfused opens, one the other way
+    round.  Returns {True: t, False: t} keyed by the FUSED decision."""
+    rng = np.random.default_rng(seed)
+    found = {}
+    f = np.float32
+    for _ in range(tries):
+        ty, tz = f(rng.uniform(0.3, 1.7)), f(rng.uniform(0.3, 1.7))
+        dy, dz = float(ty) - 1.0, float(tz) - 1.0
+        tx = f(5.0 - np.sqrt(16.0 - dy * dy - dz * dz))
+        for _ in range(6):
+            tx = np.nextafter(tx, f(-np.inf))
+        for _ in range(13):
+            t = np.array([tx, ty, tz], f)
+            a, b = bool(opening_d2(t, True) > f(16.0)), bool(opening_d2(t, False) > f(16.0))
+            if a != b and a not in found:
+                found[a] = t
+            tx = np.nextafter(tx, f(np.inf))
+        if len(found) == 2:
+            return found
+    raise AssertionError("no fma-sensitive target found")

@@ -130,3 +130,64 @@ def test_error_shrinks_with_theta_and_group_rule_is_tighter(cfg1):
         assert c32[0] + c32[1] > c1[0] + c1[1]
         assert prev is None or e1 < prev
         prev = e1
+
+
+# ---- the opening test itself, on its threshold (reading O5 / Q1 of PAPER.md:153: "strict; equality opens", and the
+# fp32 operation order d2 = fma(dz,dz, fma(dy,dy, fl(dx dx))), fl(s^2) < fl(fl(theta^2) d2)) -------------------------
+from helpers import fma_sensitive_targets, opening_case, opening_d2
+
+
+def _pair_cell_decision(t):
+    """Does the oracle's group 0 accept the level-2 cell of the pair (helpers.opening_case)?  Also checks that the
+    whole interaction list equals the independently written list builder's."""
+    pos, mom, ia, ib = opening_case(t)
+    tree = oracle.Tree(pos)
+    tree.moments(mom)
+    _, perm = tree.keys()
+    slot = {int(c): s for s, c in enumerate(perm)}
+    sa, sb = sorted((slot[ia], slot[ib]))
+    assert (sa, sb) == (32, 33)                              # group 0 = the 32 particles of octant 0
+    nd = tree.nodes()
+    om = tree.moments(mom)
+    cell = [i for i in range(tree.n_nodes) if nd["level"][i] == 2 and nd["first"][i] == 32 and nd["count"][i] == 2]
+    assert len(cell) == 1 and not nd["is_leaf"][cell[0]]
+    assert np.array_equal(om["cen"][cell[0]], np.array([5, 1, 1], np.float32))     # the centre is exact
+    cells, parts = tree.group_lists(0.5, 32, 0)
+    accepted = cell[0] in set(int(c) for c in cells)
+    assert accepted != ({32, 33} <= set(int(p) for p in parts))                    # either the cell or its two particles
+    lists, *_ = _build_lists(pos, mom, 0.5, 32, 1)
+    g0, g1, bcells, bparts = lists[0]
+    assert sorted((int(nd["level"][c]), int(nd["prefix"][c])) for c in cells) == sorted(bcells)
+    assert sorted(int(p) for p in parts) == sorted(bparts)
+    # the counters of the evaluation agree with the lists (32 members per accepted cell, self term excluded)
+    _, _, cnt = tree.eval(0.5, 32, groups=[0])
+    assert cnt[0] == 32 * len(cells) and cnt[1] == 32 * len(parts) - 32
+    return accepted
+
+
+def test_opening_test_equality_opens():
+    """t = (1, 1, 1): d = 4 = 2 s_2 exactly, fl(s^2) = 4 = fl(theta^2 d2).  The test is STRICT: equality opens."""
+    assert float(opening_d2([1, 1, 1])) == 16.0
+    assert _pair_cell_decision([1.0, 1.0, 1.0]) is False
+
+
+def test_opening_test_one_ulp_beyond_accepts():
+    """The neighbouring target whose dx is one fp32 step longer (4 + 2^-21): d2 = 16 + 2^-18, rhs = 4 + 2^-20 > 4."""
+    t = [1.0 - 2.0 ** -21, 1.0, 1.0]
+    assert float(opening_d2(t)) == 16.0 + 2.0 ** -18
+    assert _pair_cell_decision(t) is True
+    # and one step short of the threshold (dx = 4 - 2^-22, d2 < 16) opens
+    t = [1.0 + 2.0 ** -22, 1.0, 1.0]
+    assert float(opening_d2(t)) < 16.0
+    assert _pair_cell_decision(t) is False
+
+
+def test_opening_test_uses_the_fused_order():
+    """Two targets (seeded search, helpers.fma_sensitive_targets) on which d2 in the order of reading O5 and d2 as
+    three rounded squares added left to right fall on different sides of the threshold: the oracle must decide as the
+    fused order does, in both directions."""
+    found = fma_sensitive_targets()
+    for fused_accepts, t in found.items():
+        assert bool(opening_d2(t, True) > 16.0) == fused_accepts
+        assert bool(opening_d2(t, False) > 16.0) != fused_accepts
+        assert _pair_cell_decision(t) is fused_accepts
