@@ -68,7 +68,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -79,14 +79,22 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
-    def stop(self, t0, t1):
+    def started(self):
+        return self.proc is not None
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+
+    def summary(self, t0, t1):
+        """Median, minimum and count of the SM-clock samples taken between the wall-clock times t0 and t1, and every
+        throttle reason seen in them.  The sampler keeps running (stop() ends it)."""
         if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+            return {"sm_mhz": None, "sm_min_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
-        self.proc.terminate()
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ts, line in self.rows:
+        for ts, line in list(self.rows):
             f = [x.strip() for x in line.split(",")]
             if len(f) < 7:
                 continue
@@ -99,8 +107,8 @@ class ClockSampler:
                             reasons.add(nm)
             except ValueError:
                 continue
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_min_mhz": min(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
 def _workload(n, seed, cfg=3):
@@ -177,14 +185,26 @@ def job_rate(world, units_per_rank, ms):
     return world * units_per_rank / (ms * 1e-3)
 
 
+GROUP_W = 32      # targets per walk group (FF_OPT_GROUP / the oracle's W) of the headline, in BOTH arms
+NLEAF = 1         # leaf capacity of the headline, in both arms
+
+
+def _config_dict(c, world):
+    """The `config` object of the JSON line.  One function for the product arm and the reference arm, so that the two
+    lines carry the same keys and values for the same workload."""
+    return {"workload": _describe(c), "N": c["N"], "theta": c["theta"], "group": GROUP_W, "nleaf": NLEAF,
+            "l2": "GPU arm: flushed between timed steps (512 MB memset); CPU reference arm: not applicable",
+            "replicas": world, "sharding": "independent replicas, no collective"}
+
+
 def _describe(c):
     kind = {1: "hard-sphere dipoles (d=1), phi=0.05, isotropic unit moments",
             2: "hard-sphere dipoles (d=1), phi=0.1, von Mises-Fisher moments about +z (kappa=5)",
             3: "hard-sphere dipoles (d=1), phi=0.1, isotropic unit moments",
             4: "straight head-to-tail chains of 32 touching spheres within 15 deg of z, moments along the chain",
             5: "hard-sphere dipoles (d=1), phi=0.2, isotropic unit moments"}[c["config"]]
-    return ("config %d of BASELINE.json: N=%d %s, theta=%g, group rule W=32, tree rebuilt every step, H and F"
-            % (c["config"], c["N"], kind, c["theta"]))
+    return ("config %d of BASELINE.json: N=%d %s, theta=%g, group rule W=%d, tree rebuilt every step, H and F"
+            % (c["config"], c["N"], kind, c["theta"], GROUP_W))
 
 
 def _oracle_step(c, groups, nthreads=0):
@@ -196,7 +216,7 @@ def _oracle_step(c, groups, nthreads=0):
     t1 = time.perf_counter()
     t.moments(c["mom"])
     t2 = time.perf_counter()
-    t.eval(c["theta"], 32, groups=groups, nthreads=nthreads)
+    t.eval(c["theta"], GROUP_W, groups=groups, nthreads=nthreads)
     t3 = time.perf_counter()
     return t1 - t0, t2 - t1, t3 - t2
 
@@ -245,7 +265,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * step_s, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": _describe(c), "N": c["N"], "theta": c["theta"]},
+        "config": _config_dict(c, args.gpus),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "wall_s": wall, "measured_s_per_step": float(np.mean([d["measured_s"] for d in steps])),
@@ -351,6 +371,9 @@ def run_ours(args):
         ctx.build_tree(pos)
         ctx.eval_bh(pos, mom, H, F)
 
+    sampler = ClockSampler(local)          # one nvidia-smi sampler (20 ms period) for the whole run, rank 0 only
+    t_run0 = time.time()
+
     def timed(step_fn, steps, sample_clocks):
         """W >= 3 untimed steps, then `steps` steps timed on the device (CUDA events around each, L2 flushed before
         each and outside the timed region), barrier + synchronize on both sides, max over ranks."""
@@ -362,9 +385,8 @@ def run_ours(args):
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
-        sampler = ClockSampler(local)
-        if sample_clocks and rank == 0:
-            sampler.start()
+        if sample_clocks and rank == 0 and not sampler.started():
+            sampler.start()                                # keeps running until the line is printed (whole-run clocks)
             time.sleep(0.25)
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         ph = {k: 0.0 for k in ff.PHASES}
@@ -385,7 +407,7 @@ def run_ours(args):
             dist.barrier()
         ms = [a.elapsed_time(b) for a, b in ev]
         total = max_over_ranks(sum(ms), world, dev)
-        clk = sampler.stop(t_wall0, t_wall1) if (sample_clocks and rank == 0) else None
+        clk = sampler.summary(t_wall0, t_wall1) if (sample_clocks and rank == 0) else None
         return total / steps, ms, {k: v / steps for k, v in ph.items()}, n_launch, clk
 
     # interaction counts of this workload (separate, untimed run of the counting kernel variant)
@@ -763,9 +785,7 @@ def run_ours(args):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": _describe(c),
-                   "N": N, "theta": theta, "group": 32, "nleaf": 1, "l2": "flushed between timed steps (512 MB memset)",
-                   "replicas": world, "sharding": "independent replicas, no collective"},
+        "config": _config_dict(c, world),
         "clocks": clocks, "gpu_launches": int(launches), "launches_per_step": launches / args.steps,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 12, "d2h_bytes_per_step": 2 * N * 12,
                 "steps": e2e_steps, "api": "ff_eval_bh_host_async + ff_host_sync (pinned host buffers, steps pipelined over three "
@@ -786,6 +806,11 @@ def run_ours(args):
     if strong is not None:
         out["strong"] = strong
     out.update(extras)
+    if rank == 0:
+        # the same sampler over everything this invocation ran after the warm-up (timed steps, e2e, md_100_steps, the
+        # other configs, the all-pairs run, the probes): sample count, median and minimum SM clock, reasons seen
+        out["clocks"]["whole_run"] = sampler.summary(t_run0, time.time())
+        sampler.stop()
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -224,7 +224,9 @@ int ff_eval_direct_host(ff_ctx* ctx, const float* pos_host, const float* mom_hos
  * counter-based generator keyed by (seed, step_index, particle, component).
  * Streams: the call is ordered on the context's stream like every other call (work enqueued on that stream after
  * ff_step returns sees the updated state).  Internally the Lennard-Jones pass, which needs the tree but not the
- * fields, runs on a second, low-priority stream of the context beside the tree walk; the update waits for both.
+ * fields, runs on a second stream of the context beside the tree walk (same priority as the caller's stream on
+ * current GPUs: how far the two overlap depends on submission timing); the update waits for both.  All parameter
+ * checks run before anything is enqueued: a call that returns FF_ERR_INVALID_ARG has launched nothing.
  */
 typedef struct ff_step_params {
     float dtau;          /* time step (paper: 0.001) */
@@ -285,13 +287,16 @@ typedef struct ff_tree_view {
     const int32_t* leaf_count; /* [n] defined at the first slot of multi-particle leaves */
     const float* cell_centre;  /* [n_cells][4] rho'.xyz (fp32), fl(s_l^2); valid after ff_eval_bh */
     const float* cell_moment;  /* [n_cells][4] u'.xyz (fp32), N' as float; valid after ff_eval_bh */
-    const float* cell_quad;    /* [n_cells][8] FF_OPT_CELL_ORDER = 1 only (else NULL): symmetric part of the cell tensor D,
-                                  xx yy zz xy xz yz 0 0 (fp32); valid after ff_eval_bh */
+    const float* cell_quad;    /* [n_cells][8] symmetric part of the cell tensor D, xx yy zz xy xz yz 0 0 (fp32).  Non-NULL only
+                                  if the last ff_eval_bh on this tree ran with FF_OPT_CELL_ORDER = 1 (NULL before any
+                                  evaluation and after an order-0 one: the array would hold stale tensors) */
 } ff_tree_view;
 
 int ff_get_tree(ff_ctx* ctx, ff_tree_view* out);
 
-/* CUDA-event milliseconds per phase of the calls since the last ff_get_timings (needs FF_OPT_TIMING). */
+/* CUDA-event milliseconds per phase of the calls since the last ff_get_timings (needs FF_OPT_TIMING).  After ff_step
+ * with a Lennard-Jones force, FF_PH_WALK and FF_PH_STEP include whatever of the concurrent Lennard-Jones kernels ran
+ * inside their event brackets (second stream). */
 int ff_get_timings(ff_ctx* ctx, float ms[FF_N_PHASES]);
 
 /*
@@ -304,7 +309,7 @@ int ff_get_counters(ff_ctx* ctx, uint64_t* n_cell, uint64_t* n_particle, uint64_
 
 /*
  * How many of the n_mac_tests of the last ff_eval_bh the walk's cheap pre-filter (group bounding box +
- * eight probe members) could not decide and passed on to the full 32-member test
+ * four probe members) could not decide and passed on to the full 32-member test
  * (needs FF_OPT_COUNTERS).  A measurement aid: the decisions themselves are unaffected.
  */
 int ff_get_prefilter_count(ff_ctx* ctx, uint64_t* n_parked);

@@ -100,7 +100,10 @@ extern "C" int ff_create(ff_ctx** out, int64_t N, float theta, void* workspace, 
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->in_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->out_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) {
-        int least = 0, greatest = 0;                       // the lowest priority: the walk's blocks go first
+        // a second stream at the lowest priority the device offers.  On current NVIDIA parts that value is the one
+        // every default-priority stream has as well (the caller's stream included), so nothing here puts the walk's
+        // blocks first: how much of the Lennard-Jones pass lands in the walk's drain is a matter of submission timing
+        int least = 0, greatest = 0;
         e = cudaDeviceGetStreamPriorityRange(&least, &greatest);
         if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&c->lj_stream, cudaStreamNonBlocking, least);
     }
@@ -209,6 +212,7 @@ extern "C" int ff_eval_bh_range(ff_ctx* c, const float* pos, const float* mom, f
     if ((rc = ff_launch_moments(c, mom)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_MOMENTS);
     c->moments_valid = 1;
+    c->moments_order = c->order;
     ff_phase_begin(c, FF_PH_WALK);
     if ((rc = ff_launch_walk(c, H_out, F_out, (int)group_begin, (int)group_end)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_WALK);
@@ -301,11 +305,14 @@ extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* ang
     ff_device_guard guard(c);
     if (!c || !pos || !vel || !mom || !angvel || !p || n <= 0 || n > c->N) return FF_ERR_INVALID_ARG;
     if (!(p->dtau > 0.0f)) return FF_ERR_INVALID_ARG;
+    // every parameter check comes before the first launch: a refused call enqueues nothing and leaves the context as it was
+    const bool lj = p->lj_epsilon != 0.0f;
+    if (lj && (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
+    if (p->wall_epsilon != 0.0f && (!(p->lj_cutoff > 0.0f) || !(p->wall_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
     int rc;
     FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[0], 0));   // a pending download of an earlier *_host_async call
     if (p->all_pairs) {
         // the paper's All-Pairs step (Algorithm 1): h^dip, f^dip and f^sr in one pair loop, no tree
-        if (p->lj_epsilon != 0.0f && (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
         c->n = n;
         ff_phase_begin(c, FF_PH_DIRECT);
         if ((rc = ff_launch_direct(c, pos, mom, n, c->stage_H, c->stage_F, p->lj_epsilon, p->lj_sigma, p->lj_cutoff)) != FF_OK)
@@ -317,20 +324,22 @@ extern "C" int ff_step(ff_ctx* c, float* pos, float* vel, float* mom, float* ang
         c->tree_built = 0;
         return FF_OK;
     }
-    // The Lennard-Jones pass needs the tree (sorted keys and positions), not the fields: it is enqueued on its own
-    // low-priority stream AFTER the walk and runs beside it, in the SMs the persistent walk leaves idle while it drains
-    // (about 0.17 ms at N = 2^20, profiles/r2_walk_full.md); the update waits for both.
-    const bool lj = p->lj_epsilon != 0.0f;
-    if (lj && (!(p->lj_cutoff > 0.0f) || !(p->lj_sigma > 0.0f))) return FF_ERR_INVALID_ARG;
+    // The Lennard-Jones pass needs the tree (sorted keys and positions), not the fields: it is enqueued on a second
+    // stream AFTER the walk and can run beside it, in the SMs the persistent walk leaves idle while it drains
+    // (about 0.17 ms at N = 2^20, profiles/r2_walk_full.md); the update waits for both.  (No priority separates the
+    // two streams, see ff_create.)
     if ((rc = ff_build_tree(c, pos, n)) != FF_OK) return rc;
     if (lj) FF_CUDA(c, cudaEventRecord(c->ev_tree, c->stream));
     if ((rc = ff_eval_bh(c, pos, mom, c->stage_H, c->stage_F)) != FF_OK) return rc;
     ff_phase_begin(c, FF_PH_STEP);
     if (lj) {
         FF_CUDA(c, cudaStreamWaitEvent(c->lj_stream, c->ev_tree, 0));
-        if ((rc = ff_launch_lj(c, n, p, c->lj_stream)) != FF_OK) return rc;
+        rc = ff_launch_lj(c, n, p, c->lj_stream);
+        // also when the pass failed part-way: whatever it did enqueue reads the sorted keys and positions, and the
+        // caller's stream must not start the next tree build (which overwrites them) before that has drained
         FF_CUDA(c, cudaEventRecord(c->ev_lj, c->lj_stream));
         FF_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_lj, 0));
+        if (rc != FF_OK) return rc;
     }
     if ((rc = ff_launch_integrate(c, pos, vel, mom, angvel, n, p, step_index, lj)) != FF_OK) return rc;
     ff_phase_end(c, FF_PH_STEP);
@@ -364,7 +373,9 @@ extern "C" int ff_get_tree(ff_ctx* c, ff_tree_view* out)
     out->cell_first = c->cell_first; out->cell_end = c->cell_end; out->cell_level = c->cell_level;
     out->child = c->cell_child; out->leaf_count = c->leaf_count;
     out->cell_centre = (const float*)c->cell_centre; out->cell_moment = (const float*)c->cell_moment;
-    out->cell_quad = c->order == 1 ? (const float*)c->cell_quad : nullptr;
+    // only if the moments of THIS tree were computed at order 1: after an order-0 evaluation, or before any, the array
+    // holds an earlier tree's tensors or nothing
+    out->cell_quad = (c->moments_valid && c->moments_order == 1) ? (const float*)c->cell_quad : nullptr;
     return FF_OK;
 }
 

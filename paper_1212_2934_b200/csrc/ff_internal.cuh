@@ -81,6 +81,7 @@ struct ff_ctx {
                               // completed ff_build_tree (ff_k_build resets it for the next one), cleared while one runs
     const float* tree_pos;    // the pos array the current tree was built from (ff_eval_bh checks it is given the same one)
     int moments_valid;
+    int moments_order;        // the FF_OPT_CELL_ORDER the current cell data was computed with (cell_quad is defined iff 1)
     int device;
     int num_sms;
     int group;                // targets per walk group W: 32 or 64 (FF_OPT_GROUP)
@@ -91,8 +92,8 @@ struct ff_ctx {
     // buffers and events double-buffered by call parity (ff_api.cu)
     cudaStream_t in_stream, out_stream;
     cudaEvent_t ev_pos[2], ev_in[2], ev_done[2], ev_out[2];
-    // ff_step: the Lennard-Jones pass needs the tree only, not the walk's results; it runs on its own low-priority
-    // stream beside the walk and fills the SMs the draining walk leaves idle (ff_api.cu)
+    // ff_step: the Lennard-Jones pass needs the tree only, not the walk's results; it runs on a second
+    // stream beside the walk and can fill the SMs the draining walk leaves idle (ff_api.cu)
     cudaStream_t lj_stream;
     cudaEvent_t ev_tree, ev_lj;
     uint64_t host_seq;                // *_host calls issued so far

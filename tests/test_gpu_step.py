@@ -70,8 +70,12 @@ def _oracle_step(x, v, u, w, theta, kw):
     return out, (H, F, Q, fsr)
 
 
-def _check_step(before, after, ref, aux, kw):
-    """Compare through the increments, which is where the arithmetic of the step sits."""
+def _check_step(before, after, ref, aux, kw, subtract_rep=True):
+    """Compare through the increments, which is where the arithmetic of the step sits.
+
+    subtract_rep=False gates the RAW error (nothing taken off): for states that start at rest, where the representation
+    term below vanishes and the tolerance applies to the arithmetic of the step alone.  Returns, for the record, the raw
+    maximum errors and the largest share of the gate the subtraction absorbed."""
     x0, v0, u0, w0 = [a.astype(np.float64) for a in before]
     x1, v1, u1, w1 = [a.astype(np.float64) for a in after]
     xr, vr, ur, wr = ref
@@ -90,18 +94,31 @@ def _check_step(before, after, ref, aux, kw):
     scale = np.maximum(np.linalg.norm(acc_ref, axis=1), Q[:, 1] / 8.0)
     if fsr is not None:
         scale = np.maximum(scale, np.linalg.norm(fsr, axis=1) / 8.0)
-    rep = ulp * np.linalg.norm(v1, axis=1) / dt
-    err = np.maximum(np.linalg.norm(acc_gpu - acc_ref, axis=1) - rep, 0.0) / scale
+    rep = ulp * np.linalg.norm(v1, axis=1) / dt if subtract_rep else np.zeros(len(v1))
+    raw = np.linalg.norm(acc_gpu - acc_ref, axis=1)
+    err = np.maximum(raw - rep, 0.0) / scale
     assert err.max() <= TOL_STEP, err.max()
+    # the same gate written on the raw error, row by row, so that what the subtraction absorbs is visible: the raw
+    # error may exceed the tolerance only by that row's own representation term
+    assert (raw <= rep + TOL_STEP * scale).all()
     # angular-velocity increment / dtau = 5/2 (u x h - Gamma_r omega)
     t_gpu, t_ref = (w1 - w0) / dt, (wr - w0) / dt
     tscale = np.maximum(np.linalg.norm(t_ref, axis=1), 2.5 * Q[:, 0] / 8.0)
-    trep = ulp * np.linalg.norm(w1, axis=1) / dt
-    terr = np.maximum(np.linalg.norm(t_gpu - t_ref, axis=1) - trep, 0.0) / tscale
+    trep = ulp * np.linalg.norm(w1, axis=1) / dt if subtract_rep else np.zeros(len(w1))
+    traw = np.linalg.norm(t_gpu - t_ref, axis=1)
+    terr = np.maximum(traw - trep, 0.0) / tscale
     assert terr.max() <= TOL_STEP, terr.max()
+    assert (traw <= trep + TOL_STEP * tscale).all()
     # moments: unit length, and the same direction as the oracle's
     assert np.abs(np.linalg.norm(u1, axis=1) - 1.0).max() <= 4 * ulp
     assert np.abs(u1 - ur).max() <= 8 * ulp
+    # how much the subtraction absorbed is reported, not hidden (pytest -s / -rP shows it); the from-rest test below is
+    # the one where it absorbs nothing
+    stats = dict(raw_acc=float((raw / scale).max()), raw_torque=float((traw / tscale).max()),
+                 gated_acc=float(err.max()), gated_torque=float(terr.max()),
+                 rep_share_acc=float((rep / scale).max() / TOL_STEP), rep_share_torque=float((trep / tscale).max() / TOL_STEP))
+    print("step parity:", stats)
+    return stats
 
 
 KW = dict(dtau=1e-3, gamma_d=0.7, gamma_r=1.3, h_ext=(0.0, 0.1, 0.4), eps=0.5, sigma=1.0, cutoff=2.5)
@@ -126,6 +143,50 @@ def test_one_step_matches_oracle(ff, cfg_id, N):
     _check_step((x, v, u, w), after, ref, aux, KW)
     # the short-range force is not trivially zero in this test
     assert np.linalg.norm(aux[3], axis=1).max() > 0.1
+
+
+@pytest.mark.parametrize("all_pairs", [False, True])
+def test_step_from_rest_gates_the_arithmetic_alone(ff, all_pairs):
+    """v = omega = 0 at the start: the new velocities are dtau x (force), stored with a relative 2^-24, so the
+    representation term of _check_step is ~6e-8 of the force and nothing is subtracted: the 1e-4 gate applies to the raw
+    error of the step's arithmetic (Barnes-Hut or all-pairs field and force, Eq. 13, the update)."""
+    N = 3000
+    x, _, u, _ = _state(1, N, 5)
+    v, w = np.zeros_like(x), np.zeros_like(x)
+    kw = dict(KW, all_pairs=all_pairs)
+    ctx = ff.FFContext(N, 0.5)
+    dx, dv, du, dw = _dev(x), _dev(v), _dev(u), _dev(w)
+    ctx.step(dx, dv, du, dw, _params(ff, **kw), 0)
+    after = [t.cpu().numpy() for t in (dx, dv, du, dw)]
+    ref, aux = _oracle_step(x, v, u, w, 0.5, kw)
+    stats = _check_step((x, v, u, w), after, ref, aux, kw, subtract_rep=False)
+    assert stats["rep_share_acc"] == 0.0 and stats["gated_acc"] == stats["raw_acc"]
+
+
+def test_refused_parameters_enqueue_nothing(ff):
+    """Every parameter check of ff_step runs before its first launch (tree path and all-pairs path): a refused call
+    leaves the state arrays and the context's launch count as they were."""
+    import torch
+    N = 512
+    x, v, u, w = _state(1, N, 9)
+    ctx = ff.FFContext(N, 0.5)
+    for bad in (dict(wall_eps=1.0, wall_sigma=0.0, wall_lo=(0, 0, 0), wall_hi=(90, 90, 90)),
+                dict(wall_eps=1.0, wall_sigma=0.5, cutoff=0.0, eps=0.0, wall_lo=(0, 0, 0), wall_hi=(90, 90, 90)),
+                dict(eps=0.5, sigma=0.0), dict(eps=0.5, cutoff=-1.0), dict(dtau=0.0)):
+        for all_pairs in (False, True):
+            kw = dict(KW, **bad, all_pairs=all_pairs)
+            dx, dv, du, dw = _dev(x), _dev(v), _dev(u), _dev(w)
+            before = ctx.launch_count()
+            with pytest.raises(ff.FFError) as err:
+                ctx.step(dx, dv, du, dw, _params(ff, **kw), 0)
+            assert err.value.code == ff.FF_ERR_INVALID_ARG
+            assert ctx.launch_count() == before, (bad, all_pairs)
+            torch.cuda.synchronize()
+            assert np.array_equal(dx.cpu().numpy(), x) and np.array_equal(dv.cpu().numpy(), v)
+    # and the context still works
+    dx, dv, du, dw = _dev(x), _dev(v), _dev(u), _dev(w)
+    ctx.step(dx, dv, du, dw, _params(ff, **KW), 0)
+    assert ctx.launch_count() > before
 
 
 def test_step_without_short_range_force_and_drag(ff):
