@@ -15,6 +15,12 @@ ff_eval_direct (split and unsplit grids), ff_eval_bh_host and ff_step with Lenna
 and all-pairs.  The hazards it is there for: the walk's shared-memory ring, stack and parked-cell queue are ordered
 by __syncwarp only, the sort's look-back by volatile status words (the paper's own build relies on atomics used as
 locks).  Prints one line per case; the summaries are kept in profiles/.
+
+    FF_CHECKED=1 python tests/sanitizer_smoke.py --full
+
+runs the tree build and the walk (counters off and on, W = 32 and 64, N_leaf 1 and 8, cell order 0 and 1) over
+configs 3 and 4 of BASELINE.json at their full size N = 2^20, i.e. with the walk's stack, ring and parked-cell queue
+at the depth the bench reaches (the bounds checked: stack <= 1024, ring <= 128, parked <= 64 entries).
 """
 import os
 import sys
@@ -71,5 +77,33 @@ def main():
                                                                if os.environ.get("FF_CHECKED") == "1" else "release build"))
 
 
+def full():
+    for cfg in (3, 4):
+        c = ffgen.config(cfg)
+        N = len(c["pos"])
+        pos, mom = torch.from_numpy(c["pos"]).cuda(), torch.from_numpy(c["mom"]).cuda()
+        for nleaf, group, order in ((1, 32, 0), (1, 64, 0), (8, 32, 0), (1, 32, 1), (8, 32, 1)):
+            ctx = ff.FFContext(N, c["theta"], nleaf=nleaf)
+            if group != 32:
+                ctx.set_option(ff.FF_OPT_GROUP, group)
+            if order:
+                ctx.set_option(ff.FF_OPT_CELL_ORDER, order)
+            ctx.build_tree(pos)
+            H, F = ctx.eval_bh(pos, mom)
+            ctx.set_option(ff.FF_OPT_COUNTERS, 1)
+            H2, F2 = ctx.eval_bh(pos, mom)
+            torch.cuda.synchronize()
+            cnt = ctx.counters()                           # raises FFError if a device-side check failed
+            ctx.timings()
+            print("config %d N=%d nleaf=%d W=%d order=%d: counters %s, finite=%s, counting variant identical=%s"
+                  % (cfg, N, nleaf, group, order, cnt, bool(torch.isfinite(H).all() and torch.isfinite(F).all()),
+                     bool(torch.equal(H, H2) and torch.equal(F, F2))))
+            assert bool(torch.isfinite(H).all() and torch.isfinite(F).all())
+            ctx.close()
+            del ctx
+    print("full size: %s; no device-side error flag was raised" % ("CHECKED build (FF_CHECK compiled in)"
+                                                                 if os.environ.get("FF_CHECKED") == "1" else "release build"))
+
+
 if __name__ == "__main__":
-    main()
+    full() if "--full" in sys.argv else main()

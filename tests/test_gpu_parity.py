@@ -215,6 +215,27 @@ def test_group_width_64(ff, N, nleaf, theta, cfg):
     assert ctx.counters() == cnt32
 
 
+def test_opening_test_on_its_threshold(ff):
+    """The crafted inputs of tests/test_oracle_walk.py (helpers.opening_case): one group, one cell, one critical member
+    whose fp32 d2 sits exactly on, one step beyond, one step short of the threshold, or where the fused and the unfused
+    order of the sum of squares decide differently.  The GPU must take the oracle's decision in every case: counters
+    equal (a wrongly accepted or opened cell changes n_cell by 32), tree bit-exact, H and F within tolerance."""
+    from helpers import fma_sensitive_targets, opening_case
+    cases = [[1.0, 1.0, 1.0], [1.0 - 2.0 ** -21, 1.0, 1.0], [1.0 + 2.0 ** -22, 1.0, 1.0]]
+    cases += [t for _, t in sorted(fma_sensitive_targets().items())]
+    n_cell = []
+    for t in cases:                      # W = 32 only: with W = 64 all 35 particles are one group and nothing is tested
+        pos, mom, _, _ = opening_case(t)
+        ctx, H, F = _gpu_bh(ff, pos, mom, 0.5)
+        Ho, Fo, cnt, otree, Q = oracle.barnes_hut(pos, mom, 0.5, 32, scale=True)
+        _check_tree(ff, ctx, otree, otree.moments(mom))
+        assert ctx.counters() == cnt, (t, ctx.counters(), cnt)
+        check_hf(H, F, Ho, Fo, Q, TOL_BH)
+        n_cell.append(cnt[0])
+    # the five cases are not the same decision five times: accepting the pair's cell adds 32 cell terms
+    assert n_cell[1] == n_cell[0] + 32 and n_cell[2] == n_cell[0] and abs(n_cell[3] - n_cell[4]) == 32
+
+
 @pytest.mark.parametrize("N,nleaf,theta,cfg", [(4096, 1, 0.5, 1), (2, 1, 0.5, 1), (33, 1, 0.7, 1), (1000, 1, 0.3, 1),
                                                 (4097, 4, 0.6, 1), (3000, 1, 0.5, 4), (2500, 16, 1.0, 2), (6000, 1, 0.8, 2)])
 def test_first_order_cell_term(ff, N, nleaf, theta, cfg):
@@ -247,6 +268,9 @@ def test_first_order_cell_term(ff, N, nleaf, theta, cfg):
     ctx.set_option(ff.FF_OPT_CELL_ORDER, 0)
     H0, _ = ctx.eval_bh(p, m)
     assert rel_err(H0.cpu().numpy(), H0o)[3] < 1e-5 and "cell_quad" not in ctx.get_tree()
+    ctx.set_option(ff.FF_OPT_CELL_ORDER, 1)
+    assert "cell_quad" not in ctx.get_tree()     # the option is set, but the cell data on the device is the order-0 evaluation's
+    ctx.set_option(ff.FF_OPT_CELL_ORDER, 0)
     with pytest.raises(ff.FFError):
         ctx.set_option(ff.FF_OPT_CELL_ORDER, 2)
     ctx.set_option(ff.FF_OPT_GROUP, 64)
@@ -484,49 +508,101 @@ def test_config2_theta_sweep(ff):
     _check_tree(ff, ctx, otree, om)
 
 
-# ------------------------------------------- full sizes, sampled oracle ----
-def _sampled_parity(ff, c, n_groups, seed=0, survey=True):
+# ------------------------------------------- full sizes ----
+def _full_size_parity(ff, c, runs=None, survey=True, nleaf=1, order=0, group=32):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (counters off), against the oracle.
+
+    runs=None: the oracle walks EVERY group; H and F of every row within tolerance, interaction counters equal.
+    runs=[(g0, g1), ...]: contiguous runs of walk groups; per run ff_eval_bh_range with counters on must report the
+    oracle's counters for exactly those groups, and the rows of the run (taken from the full, counters-off
+    evaluation) are within tolerance.  Tree: keys, permutation and (first, end, level) of every cell bit-exact."""
     pos, mom, theta = c["pos"], c["mom"], c["theta"]
     N = len(pos)
-    ctx = ff.FFContext(N, theta)
+    ctx = ff.FFContext(N, theta, nleaf=nleaf)
+    if group != 32:
+        ctx.set_option(ff.FF_OPT_GROUP, group)
+    if order:
+        ctx.set_option(ff.FF_OPT_CELL_ORDER, order)
     p, m = _dev(pos), _dev(mom)
     ctx.build_tree(p)
-    H, F = ctx.eval_bh(p, m)
-    H, F = H.cpu().numpy(), F.cpu().numpy()
-    otree = oracle.Tree(pos)
+    Hd, Fd = ctx.eval_bh(p, m)                       # counters off: the kernel variant bench.py times
+    H, F = Hd.cpu().numpy(), Fd.cpu().numpy()
+    assert np.isfinite(H).all() and np.isfinite(F).all()
+    otree = oracle.Tree(pos, nleaf)
     otree.moments(mom)
     t = ctx.get_tree()
     okey, operm = otree.keys()
     assert np.array_equal(t["key"], okey) and np.array_equal(t["perm"].astype(np.int64), operm)
     nd = otree.nodes()
-    assert t["n_cells"] == int((nd["is_leaf"] == 0).sum())
     internal = nd["is_leaf"] == 0
+    assert t["n_cells"] == int(internal.sum())
     assert np.array_equal(t["cell_first"], nd["first"][internal].astype(np.int32))
     assert np.array_equal(t["cell_end"], (nd["first"] + nd["count"])[internal].astype(np.int32))
     assert np.array_equal(t["cell_level"], nd["level"][internal])
-    groups = np.random.default_rng(seed).choice((N + 31) // 32, n_groups, replace=False)
-    Ho, Fo, _, Q = otree.eval(theta, 32, groups=groups, scale=True)
-    rows = operm[(groups[:, None] * 32 + np.arange(32)[None, :]).ravel()]
-    rows = rows[rows < N]
+    ctx.set_option(ff.FF_OPT_COUNTERS, 1)
+    if runs is None:
+        Ho, Fo, cnt, Q = otree.eval(theta, group, scale=True, order=order)
+        ctx.eval_bh(p, m, Hd, Fd)
+        assert ctx.counters() == cnt                 # identical interaction sets over all N targets
+        # every row: the term-scale metric <= tol; the survey metric <= tol on all but <= 1e-5 of the rows (one row of
+        # config 3's 2^20 sits at 1.10e-4 in F, a sum that cancels below 1/8 of its term scale; DESIGN.md section 6)
+        tail = "tail" if survey else False
+        eh, ef = check_hf(H, F, Ho, Fo, Q, TOL_BH, survey=tail)
+        print("all %d rows, counters %s: term-scale metric max H %.2e F %.2e" % (N, cnt, eh[0], ef[0]))
+        # the counting variant of the walk computes the same values
+        check_hf(Hd.cpu().numpy(), Fd.cpu().numpy(), Ho, Fo, Q, TOL_BH, survey=tail)
+        return ctx
+    n_groups = (N + group - 1) // group
+    all_rows = []
+    Ho = Fo = Q = None
+    for g0, g1 in runs:
+        assert 0 <= g0 < g1 <= n_groups
+        groups = np.arange(g0, g1)
+        Hr, Fr, cnt, Qr = otree.eval(theta, group, groups=groups, scale=True, order=order)
+        ctx.eval_bh_range(p, m, Hd, Fd, g0, g1)
+        assert ctx.counters() == cnt, (g0, g1, ctx.counters(), cnt)
+        rows = operm[g0 * group:min(N, g1 * group)]
+        if Ho is None:
+            Ho, Fo, Q = Hr, Fr, Qr
+        else:
+            Ho[rows], Fo[rows], Q[rows] = Hr[rows], Fr[rows], Qr[rows]
+        all_rows.append(rows)
+    rows = np.concatenate(all_rows)
     check_hf(H[rows], F[rows], Ho[rows], Fo[rows], Q[rows], TOL_BH, survey=survey)
-    assert np.isfinite(H).all() and np.isfinite(F).all()
-    return ctx, H, F
+    return ctx
 
 
-def test_config3_one_million_sampled(ff):
-    c = ffgen.config(3)
-    ctx, H, F = _sampled_parity(ff, c, 256)
-    # direct kernel on sampled rows only is not possible (it evaluates all targets); it is timed in bench.py
+def _spread_runs(N, group, n_runs, run_len):
+    """n_runs contiguous runs of run_len walk groups, spread evenly over the sorted order (first and last included)."""
+    n_groups = (N + group - 1) // group
+    starts = np.linspace(0, n_groups - run_len, n_runs).astype(np.int64)
+    return [(int(s0), int(s0 + run_len)) for s0 in starts]
 
 
-def test_config4_chains_sampled(ff):
+def test_config3_one_million_every_group(ff):
+    # N = 2^20, theta = 0.5: the configuration the metric is quoted on.  All 32 768 groups, counters equal.
+    _full_size_parity(ff, ffgen.config(3))
+
+
+def test_config4_chains_every_group(ff):
     # chains: the one full-size config whose sums cancel by construction (DESIGN.md section 6) -> term-scale metric only
-    _sampled_parity(ff, ffgen.config(4), 256, survey=False)
+    _full_size_parity(ff, ffgen.config(4), survey=False)
 
 
-def test_config5_sixteen_million_sampled(ff):
-    # N = 2^24, phi = 0.2, theta = 0.6: the HBM-resident case; the oracle walks 64 sampled groups
-    _sampled_parity(ff, ffgen.config(5), 64)
+def test_config5_sixteen_million_runs(ff):
+    # N = 2^24, phi = 0.2, theta = 0.6: the HBM-resident case; 4 contiguous runs of 256 groups (32 768 targets), counters per run
+    c = ffgen.config(5)
+    _full_size_parity(ff, c, runs=_spread_runs(len(c["pos"]), 32, 4, 256))
+
+
+@pytest.mark.parametrize("cfg,nleaf,order,group", [(3, 8, 0, 32), (3, 1, 1, 32), (3, 8, 1, 32), (3, 1, 0, 64),
+                                                   (4, 1, 0, 64), (4, 8, 0, 32)])
+def test_cell_variants_at_full_size(ff, cfg, nleaf, order, group):
+    """SURVEY.md 8(f4) at the one-million configs: bucket leaves, the first-order cell term, both, and W = 64, each
+    against the oracle's evaluation of the same variant on 4 contiguous runs of 64 groups with counters per run."""
+    c = ffgen.config(cfg)
+    _full_size_parity(ff, c, runs=_spread_runs(len(c["pos"]), group, 4, 64), survey=cfg != 4, nleaf=nleaf, order=order,
+                      group=group)
 
 
 @pytest.mark.gpu
@@ -541,6 +617,20 @@ def test_checked_build_raises_no_device_side_check():
                          capture_output=True, text=True, timeout=900)
     assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-2000:]
     assert "CHECKED build" in out.stdout
+
+
+@pytest.mark.gpu
+def test_checked_build_at_full_depth():
+    """The checked library over configs 3 and 4 at N = 2^20 (tests/sanitizer_smoke.py --full): the walk's stack, ring and
+    parked-queue bounds and every index check at the depth the bench reaches, for W = 32 / 64, N_leaf 1 / 8, order 0 / 1."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "tests", "sanitizer_smoke.py"), "--full"],
+                         env=dict(os.environ, FF_CHECKED="1"), cwd=root, capture_output=True, text=True, timeout=1200)
+    assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-2000:]
+    assert "full size: CHECKED build" in out.stdout and out.stdout.count("counters (") == 10
+    print(out.stdout)
 
 
 @pytest.mark.gpu
