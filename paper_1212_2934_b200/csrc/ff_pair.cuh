@@ -160,7 +160,10 @@ struct ff_accq2 {
 };
 __device__ __forceinline__ void ff_accq2_zero(ff_accq2& s) { s.gxx = s.gyy = s.gzz = s.gxy = s.gxz = s.gyz = ff_dup(0.0f); }
 
-// Q0 = Dxx, Dyy, Dzz, Dxy ; Q1 = Dxz, Dyz (a particle carries D = 0 and gets exactly nothing from this)
+// Q0 = Dxx, Dyy, Dzz, Dxy ; Q1 = Dxz, Dyz.  A particle carries D = 0: every first-order term is then exactly zero, and
+// the 49 instructions are skipped.  The ring entry, and with it this branch, is the same for all lanes that evaluate
+// it (a half-warp at W = 32); the walk appends a round's cells before its particles so that the two half-warps mostly
+// see the same kind of entry (ff_walk.cu).
 __device__ __forceinline__ void ff_pair2_quad(const float4& A, const float2& B, const float4& Q0, const float2& Q1,
                                               const ff_target2& t, ff_acc2& s, ff_accq2& sq)
 {
@@ -168,6 +171,9 @@ __device__ __forceinline__ void ff_pair2_quad(const float4& A, const float2& B, 
     ff_pair2_geom(A, t, dx, dy, dz, r2);
     const float2 rinv = ff_rsqrt2(r2);
     ff_pair2_accum(A, B, t, dx, dy, dz, rinv, s);
+    const unsigned any = __float_as_uint(Q0.x) | __float_as_uint(Q0.y) | __float_as_uint(Q0.z) | __float_as_uint(Q0.w) |
+                         __float_as_uint(Q1.x) | __float_as_uint(Q1.y);
+    if ((any << 1) == 0u) return;                                                  // D = +-0 in all six components
     const float2 rinv2 = __fmul2_rn(rinv, rinv);
     const float2 nr3 = __fmul2_rn(rinv2, make_float2(-rinv.x, -rinv.y));
     const float2 c1 = __fmul2_rn(nr3, __fmul2_rn(rinv2, ff_dup(-3.0f)));           // 3 / R^5

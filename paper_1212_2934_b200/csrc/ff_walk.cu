@@ -180,10 +180,17 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
         __syncwarp();
     };
     // append the lanes with `take` set (A = x, y, z, mx; B = my, mz) to the ring
-    auto append = [&](bool take, const float4& A, const float2& B, const float4& Q0, const float2& Q1) {
+    // (QUAD: `first` marks the accepted cells of a round; they go in front of the round's particles, so that
+    // neighbouring ring entries are of one kind and ff_pair2_quad's skip of the first-order block seldom diverges)
+    auto append = [&](bool take, const float4& A, const float2& B, const float4& Q0, const float2& Q1, bool first = false) {
         const unsigned m = __ballot_sync(FF_FULL, take);
+        int rank = __popc(m & lt);
+        if (QUAD) {
+            const unsigned mf = __ballot_sync(FF_FULL, take && first);
+            rank = first ? __popc(mf & lt) : __popc(mf) + __popc(m & ~mf & lt);
+        }
         if (take) {
-            const int slot = (pend_head + pend_cnt + __popc(m & lt)) & (FF_WALK_PEND - 1);
+            const int slot = (pend_head + pend_cnt + rank) & (FF_WALK_PEND - 1);
             sm.pendA[slot] = A;
             sm.pendB[slot] = B;
             if (QUAD) { sm.pendQ0[slot] = Q0; sm.pendQ1[slot] = Q1; }
@@ -324,7 +331,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
                 const float4 t4 = __ldg(quad + 2 * (size_t)e + 1);
                 Q1 = make_float2(t4.x, t4.y);
             }
-            append(take, make_float4(A.x, A.y, A.z, B.x), make_float2(B.y, B.z), Q0, Q1);
+            append(take, make_float4(A.x, A.y, A.z, B.x), make_float2(B.y, B.z), Q0, Q1, accept_cell);
         }
         // the children of an opened cell: the non-empty sub-cells, compacted to the front of its eight links
         int4 c0 = make_int4(-1, -1, -1, -1), c1 = c0;
