@@ -500,7 +500,8 @@ def run_ours(args):
     probes = {name: max(ctx.measure_probe(kind, 1 << 13) for _ in range(2))
               for name, kind in (("ffma", ff.FF_PROBE_FFMA), ("ffma2_three_register_pairs", ff.FF_PROBE_FFMA2_PAIRS),
                                  ("ffma2_reused_operand", ff.FF_PROBE_FFMA2_REUSE),
-                                 ("ffma2_scalar_operand", ff.FF_PROBE_FFMA2_SCALAR), ("eval_loop", ff.FF_PROBE_EVAL))}
+                                 ("ffma2_scalar_operand", ff.FF_PROBE_FFMA2_SCALAR), ("eval_loop", ff.FF_PROBE_EVAL),
+                                 ("eval_loop_scalar", ff.FF_PROBE_EVAL_SCALAR), ("eval_loop_hybrid", ff.FF_PROBE_EVAL_HYBRID))}
     roofline = {
         "bound": "alu", "kernel": "ff_k_walk", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": achieved / peak_tflops, "traffic": WALK_DRAM_TRAFFIC_BYTES, "traffic_source": WALK_DRAM_TRAFFIC_SOURCE,
@@ -512,6 +513,10 @@ def run_ours(args):
                                                                 "ffma2_scalar_operand")},
         "eval_loop_tflops": probes["eval_loop"], "eval_loop_ceiling_frac": probes["eval_loop"] / peak_tflops,
         "frac_of_eval_loop_ceiling": achieved / probes["eval_loop"],
+        # the same 36 operations per interaction in the two other encodings (csrc/ff_probe.cu): all scalar FFMA / FMUL,
+        # and packed except for the twelve three-register-pair FFMA2 (as 24 scalar FFMA).  If neither beats
+        # eval_loop_tflops the packed encoding is the fastest form of this arithmetic on this part.
+        "eval_loop_scalar_tflops": probes["eval_loop_scalar"], "eval_loop_hybrid_tflops": probes["eval_loop_hybrid"],
         "interactions_per_launch": interactions, "flop_per_interaction": FLOP_PER_INTERACTION,
         "kernel_ms": walk_ms, "kernel_share_of_step": walk_ms / ms_per_step,
         "interactions_per_s": interactions / (walk_ms * 1e-3),

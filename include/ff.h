@@ -334,14 +334,20 @@ int ff_measure_fp32_peak(ff_ctx* ctx, int iters, double* tflops);
  *   FF_PROBE_FFMA2_SCALAR  packed FFMA2 with one scalar operand in the broadcast form (how the sources enter Eq. 11-12)
  *   FF_PROBE_EVAL          the evaluation loop of the walk alone: 36 packed FP32 instructions (force as a tensor) + 2 MUFU.RSQ per source
  *                          and pair of targets on shared-memory records, 60 flop per interaction -- the ceiling of the
- *                          walk and of the direct kernel
+ *                          walk and of the direct kernel AS ENCODED in packed FP32
+ *   FF_PROBE_EVAL_SCALAR   the same 36 operations per target on scalars (72 FFMA / FMUL per source and pair of targets)
+ *   FF_PROBE_EVAL_HYBRID   packed except for the twelve FFMA2 with three different register-pair operands, which run as
+ *                          24 scalar FFMA -- together with _SCALAR the evidence for whether the packed form's operand
+ *                          bandwidth or the arithmetic bounds that loop
  */
 enum {
     FF_PROBE_FFMA = 0,
     FF_PROBE_FFMA2_PAIRS = 1,
     FF_PROBE_FFMA2_REUSE = 2,
     FF_PROBE_FFMA2_SCALAR = 3,
-    FF_PROBE_EVAL = 4
+    FF_PROBE_EVAL = 4,
+    FF_PROBE_EVAL_SCALAR = 5,
+    FF_PROBE_EVAL_HYBRID = 6
 };
 int ff_measure_probe(ff_ctx* ctx, int kind, int iters, double* tflops);
 

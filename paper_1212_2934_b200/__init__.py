@@ -28,6 +28,7 @@ FF_OPT_THETA, FF_OPT_NLEAF, FF_OPT_COUNTERS, FF_OPT_TIMING, FF_OPT_GROUP, FF_OPT
 FF_N_PHASES = 7
 PHASES = ("bbox_keys", "sort", "build", "moments", "walk", "direct", "step")
 FF_PROBE_FFMA, FF_PROBE_FFMA2_PAIRS, FF_PROBE_FFMA2_REUSE, FF_PROBE_FFMA2_SCALAR, FF_PROBE_EVAL = 0, 1, 2, 3, 4
+FF_PROBE_EVAL_SCALAR, FF_PROBE_EVAL_HYBRID = 5, 6
 FF_CHILD_EMPTY = -1
 FF_CHILD_LEAF1, FF_CHILD_MULTI, FF_CHILD_SLOT = 0x80000000, 0x40000000, 0x3FFFFFFF
 

@@ -65,6 +65,59 @@ __global__ void __launch_bounds__(FF_PROBE_THREADS) ff_k_probe_ffma2(int iters, 
 // kind 4: the evaluation loop of the walk alone -- every lane evaluates a batch of 32 shared-memory source records
 // for its two targets exactly as ff_k_walk<32> does (half-warps take the even / odd records), over and over.
 // Launched with the walk's block shape and residency (4 warps per block, FF_WALK_MINB blocks per SM).
+// MODE 0: the loop as the kernels have it (ff_pair2g: 36 packed instructions).  MODE 1: the same 36 operations per target
+// written on scalars (72 FFMA / FMUL per source and pair of targets, no packed instruction).  MODE 2: packed wherever
+// an operand is a broadcast scalar or repeats, but the twelve FFMA2 whose three operands are three different register
+// pairs (h += (p rho) a, T += (p rho) e, G += (p rho) e: 3 + 3 + 6) as 24 scalar FFMA.  Modes 1 and 2 answer whether the
+// packed form's operand bandwidth or the arithmetic itself bounds the loop.
+struct ff_probe_acc1 { float hx, hy, hz, txx, tyy, tzz, gxy, gxz, gyz; };
+
+__device__ __forceinline__ void ff_probe_pair1(const float4& A, const float2& B, float px_, float py_, float pz_,
+                                               ff_probe_acc1& s)
+{
+    const float dx = px_ - A.x, dy = py_ - A.y, dz = pz_ - A.z;
+    const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+    const float rinv = ff_rsqrt(r2);
+    const float mx = A.w, my = B.x, mz = B.y;
+    const float rinv2 = __fmul_rn(rinv, rinv);
+    const float nr3 = __fmul_rn(rinv2, -rinv);
+    const float p = __fmul_rn(nr3, __fmul_rn(rinv2, -3.0f));
+    const float a = __fmaf_rn(mz, dz, __fmaf_rn(my, dy, __fmul_rn(mx, dx)));
+    const float px = __fmul_rn(p, dx), py = __fmul_rn(p, dy), pz = __fmul_rn(p, dz);
+    s.hx = __fmaf_rn(px, a, s.hx); s.hy = __fmaf_rn(py, a, s.hy); s.hz = __fmaf_rn(pz, a, s.hz);
+    s.hx = __fmaf_rn(nr3, mx, s.hx); s.hy = __fmaf_rn(nr3, my, s.hy); s.hz = __fmaf_rn(nr3, mz, s.hz);
+    const float m = __fmul_rn(a, __fmul_rn(rinv2, -2.5f));
+    const float ex = __fmaf_rn(m, dx, mx), ey = __fmaf_rn(m, dy, my), ez = __fmaf_rn(m, dz, mz);
+    s.txx = __fmaf_rn(px, ex, s.txx); s.tyy = __fmaf_rn(py, ey, s.tyy); s.tzz = __fmaf_rn(pz, ez, s.tzz);
+    s.gxy = __fmaf_rn(px, ey, s.gxy); s.gxy = __fmaf_rn(py, ex, s.gxy);
+    s.gxz = __fmaf_rn(px, ez, s.gxz); s.gxz = __fmaf_rn(pz, ex, s.gxz);
+    s.gyz = __fmaf_rn(py, ez, s.gyz); s.gyz = __fmaf_rn(pz, ey, s.gyz);
+}
+
+#define FF_S2(acc, u, v) do { acc.x = __fmaf_rn(u.x, v.x, acc.x); acc.y = __fmaf_rn(u.y, v.y, acc.y); } while (0)
+__device__ __forceinline__ void ff_probe_pair2_hybrid(const float4& A, const float2& B, const ff_target2& t, ff_accg2& s)
+{
+    float2 dx, dy, dz, r2;
+    ff_pair2_geom(A, t, dx, dy, dz, r2);
+    const float2 rinv = ff_rsqrt2(r2);
+    const float2 mx = ff_dup(A.w), my = ff_dup(B.x), mz = ff_dup(B.y);
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 nr3 = __fmul2_rn(rinv2, make_float2(-rinv.x, -rinv.y));
+    const float2 p = __fmul2_rn(nr3, __fmul2_rn(rinv2, ff_dup(-3.0f)));
+    const float2 a = __ffma2_rn(mz, dz, __ffma2_rn(my, dy, __fmul2_rn(mx, dx)));
+    const float2 px = __fmul2_rn(p, dx), py = __fmul2_rn(p, dy), pz = __fmul2_rn(p, dz);
+    FF_S2(s.hx, px, a); FF_S2(s.hy, py, a); FF_S2(s.hz, pz, a);
+    s.hx = __ffma2_rn(nr3, mx, s.hx); s.hy = __ffma2_rn(nr3, my, s.hy); s.hz = __ffma2_rn(nr3, mz, s.hz);
+    const float2 m = __fmul2_rn(a, __fmul2_rn(rinv2, ff_dup(-2.5f)));
+    const float2 ex = __ffma2_rn(m, dx, mx), ey = __ffma2_rn(m, dy, my), ez = __ffma2_rn(m, dz, mz);
+    FF_S2(s.txx, px, ex); FF_S2(s.tyy, py, ey); FF_S2(s.tzz, pz, ez);
+    FF_S2(s.gxy, px, ey); FF_S2(s.gxy, py, ex);
+    FF_S2(s.gxz, px, ez); FF_S2(s.gxz, pz, ex);
+    FF_S2(s.gyz, py, ez); FF_S2(s.gyz, pz, ey);
+}
+#undef FF_S2
+
+template <int MODE>
 __global__ void __launch_bounds__(FF_WALK_WARPS * 32, FF_WALK_MINB)
 ff_k_probe_eval(int iters, float seed, float* __restrict__ sink)
 {
@@ -81,15 +134,27 @@ ff_k_probe_eval(int iters, float seed, float* __restrict__ sink)
     tg.uz = make_float2(0.8f, 0.6f);
     ff_accg2 s;
     ff_accg2_zero(s);
+    ff_probe_acc1 s0 = { 0, 0, 0, 0, 0, 0, 0, 0, 0 }, s1 = s0;
     for (int it = 0; it < iters; ++it) {
         const float4* pa = qa[w] + half;
         const float2* pb = qb[w] + half;
 #pragma unroll 4
-        for (int i = 0; i < 16; ++i) ff_pair2g(pa[2 * i], pb[2 * i], tg, s);
+        for (int i = 0; i < 16; ++i) {
+            if (MODE == 0) ff_pair2g(pa[2 * i], pb[2 * i], tg, s);
+            else if (MODE == 2) ff_probe_pair2_hybrid(pa[2 * i], pb[2 * i], tg, s);
+            else {
+                const float4 A = pa[2 * i];
+                const float2 B = pb[2 * i];
+                ff_probe_pair1(A, B, tg.px.x, tg.py.x, tg.pz.x, s0);
+                ff_probe_pair1(A, B, tg.px.y, tg.py.y, tg.pz.y, s1);
+            }
+        }
         __syncwarp();
     }
-    const float r = s.hx.x + s.hx.y + s.hy.x + s.hy.y + s.hz.x + s.hz.y + s.txx.x + s.txx.y + s.tyy.x + s.tyy.y + s.tzz.x +
-                    s.tzz.y + s.gxy.x + s.gxy.y + s.gxz.x + s.gxz.y + s.gyz.x + s.gyz.y;
+    float r = s.hx.x + s.hx.y + s.hy.x + s.hy.y + s.hz.x + s.hz.y + s.txx.x + s.txx.y + s.tyy.x + s.tyy.y + s.tzz.x +
+              s.tzz.y + s.gxy.x + s.gxy.y + s.gxz.x + s.gxz.y + s.gyz.x + s.gyz.y;
+    r += s0.hx + s0.hy + s0.hz + s0.txx + s0.tyy + s0.tzz + s0.gxy + s0.gxz + s0.gyz;
+    r += s1.hx + s1.hy + s1.hz + s1.txx + s1.tyy + s1.tzz + s1.gxy + s1.gxz + s1.gyz;
     if (r == 12345.678f) sink[0] = r;
 }
 
@@ -117,12 +182,14 @@ int ff_launch_probe(ff_ctx* c, int kind, int iters, double* tflops)
     float ms = 0.f;
     int rc;
     double flop;
-    if (kind == FF_PROBE_EVAL) {
+    if (kind == FF_PROBE_EVAL || kind == FF_PROBE_EVAL_SCALAR || kind == FF_PROBE_EVAL_HYBRID) {
+        void (*kernel)(int, float, float*) = kind == FF_PROBE_EVAL ? ff_k_probe_eval<0>
+                                           : kind == FF_PROBE_EVAL_SCALAR ? ff_k_probe_eval<1> : ff_k_probe_eval<2>;
         int per_sm = 0;
-        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ff_k_probe_eval, FF_WALK_WARPS * 32, 0));
+        FF_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, FF_WALK_WARPS * 32, 0));
         per_sm = max(1, min(per_sm, FF_WALK_MINB));
         const int blocks = c->num_sms * per_sm;
-        if ((rc = ff_time_probe(c, ff_k_probe_eval, blocks, FF_WALK_WARPS * 32, iters, sink, &ms)) != FF_OK) return rc;
+        if ((rc = ff_time_probe(c, kernel, blocks, FF_WALK_WARPS * 32, iters, sink, &ms)) != FF_OK) return rc;
         // per warp and iteration: 32 records x 32 targets = 1024 interactions of 60 flop
         flop = 60.0 * 1024.0 * (double)iters * FF_WALK_WARPS * (double)blocks;
     } else {
