@@ -34,6 +34,9 @@
 #ifndef FF_WALK_MINB
 #define FF_WALK_MINB 5             // min resident blocks per SM asked of ptxas (caps registers at 96; 5 x 4 warps per SM)
 #endif
+#ifndef FF_WALK_MINB_QUAD
+#define FF_WALK_MINB_QUAD 4        // the same for the order-1 walk: 119 registers at 4; 5 (95 registers, no spills) measured slower, DESIGN.md 8b
+#endif
 #define FF_WALK_STACK 1024         // traversal stack entries per warp
 #ifndef FF_WALK_BATCH
 #define FF_WALK_BATCH 64           // ring entries evaluated in one go

@@ -457,7 +457,7 @@ ff_walk_group(ff_walk_smem<W, QUAD>& sm, const int grp, const int lane,
 // zeroed by the last cell-moment launch), so no SM idles while one block's slowest group finishes
 // and consecutive (spatially adjacent) groups run at the same time and share cells in L1/L2.
 template <int W, bool COUNT, bool BUCKET, bool QUAD>
-__global__ void __launch_bounds__(FF_WALK_WARPS * 32, QUAD ? 4 : FF_WALK_MINB)
+__global__ void __launch_bounds__(FF_WALK_WARPS * 32, QUAD ? FF_WALK_MINB_QUAD : FF_WALK_MINB)
 ff_k_walk(int n, int group_begin, int group_end, float theta, ff_globals* __restrict__ g, const float4* __restrict__ pos_s,
           const float4* __restrict__ mom_s, const uint32_t* __restrict__ perm,
           const int4* __restrict__ cell_info, const int4* __restrict__ cell_child,
